@@ -1,0 +1,121 @@
+"""Pins against values the paper prints: the 20 MMS errors of Tables 3-7,
+reproduced (a) in closed form for every N and (b) by actually running the oracle at N = 128;
+plus second-order convergence (eq. 15) for all 27 boundary-condition combinations.
+
+Closed form (R18): for an eigenfunction manufactured solution u = prod g_d(w_d x_d),
+f = -(sum w_d^2) u, the discrete solution is u_h = u * sum w_d^2 / sum ((2/h) sin(w_d h/2))^2,
+hence ||e||_rms = |1 - sum w^2 / sum((2/h) sin(w h/2))^2| * rms(u), with h = pi/N."""
+import itertools
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import poisson_oracle as po
+from paper_1909_05423_b200 import workloads as wl
+
+P, N, D = po.PERIODIC, po.NEUMANN, po.DIRICHLET
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "paper_tables_3_7.txt")
+
+
+def read_tables():
+    rows = []
+    with open(GOLDEN) as fh:
+        for line in fh:
+            if line.startswith("#") or not line.strip():
+                continue
+            t = line.split()
+            rows.append(dict(table=int(t[0]), bc=wl.parse_bc("".join(t[1:4])), N=int(t[4]), err=float(t[5]),
+                             omega=tuple(int(v) for v in t[6:9]), src=t[9]))
+    return rows
+
+
+def closed_form_error(bc, n, omega):
+    h = math.pi / n
+    s_cont = sum(w * w for w in omega)
+    s_disc = sum(((2 / h) * math.sin(w * h / 2)) ** 2 for w in omega)
+    n_periodic = sum(1 for b in bc if b == P)          # complex exponentials have |g| = 1
+    rms_u = math.sqrt(0.5) ** (3 - n_periodic)
+    return abs(1 - s_cont / s_disc) * rms_u
+
+
+@pytest.mark.parametrize("row", read_tables(), ids=lambda r: f"T{r['table']}-N{r['N']}")
+def test_printed_errors_closed_form(row):
+    e = closed_form_error(row["bc"], row["N"], row["omega"])
+    # printed to 6 significant digits: agree to 0.6 units of the sixth digit
+    assert abs(e - row["err"]) <= 0.6 * 10 ** (math.floor(math.log10(row["err"])) - 5), (e, row)
+
+
+def mms_complex_periodic(bc, n, omega):
+    """Real and imaginary parts of u = prod g_d on a length-pi domain, g = exp(i w x) on
+    periodic axes, cos on Neumann, sin on Dirichlet.  Returns a list of
+    (f, u) real pairs whose errors add in quadrature (R17: complex sources = two solves)."""
+    h = math.pi / n
+    x = (np.arange(n) + 0.5) * h
+    facs = []
+    for b, w in zip(bc, omega):
+        if b == P:
+            facs.append(np.exp(1j * w * x))
+        elif b == N:
+            facs.append(np.cos(w * x) + 0j)
+        else:
+            facs.append(np.sin(w * x) + 0j)
+    gx, gy, gz = facs
+    u = gz[:, None, None] * gy[None, :, None] * gx[None, None, :]
+    f = -sum(w * w for w in omega) * u
+    parts = [(f.real, u.real)]
+    if any(b == P for b in bc):
+        parts.append((f.imag, u.imag))
+    return parts, (h, h, h)
+
+
+@pytest.mark.parametrize("table", [3, 4, 5, 6, 7])
+def test_printed_errors_by_solving_at_128(table):
+    row = [r for r in read_tables() if r["table"] == table and r["N"] == 128][0]
+    parts, h = mms_complex_periodic(row["bc"], 128, row["omega"])
+    sq = 0.0
+    for f, u in parts:
+        uh = po.solve(f, h, row["bc"])
+        if po.is_singular(row["bc"]):
+            u = u - u.mean()
+        sq += np.mean((uh - u) ** 2)
+    e = math.sqrt(sq)
+    assert abs(e - row["err"]) <= 1e-5 * row["err"], (e, row["err"])
+
+
+@pytest.mark.parametrize("bc", list(itertools.product((P, N, D), repeat=3)),
+                         ids=lambda bc: "".join(po.BC_NAMES[b] for b in bc))
+def test_second_order_convergence_all_27(bc):
+    """Error ratio 4 +- 0.3 on grid halving (north_star), unit cube, workloads.mms."""
+    errs = []
+    for n in (8, 16, 32):
+        shape, h = (n, n, n), (1.0 / n,) * 3
+        f, u, _ = wl.mms(shape, h, bc, omega=(1, 1, 1))
+        uh = po.solve(f, h, bc)
+        if po.is_singular(bc):
+            u = u - u.mean()
+        errs.append(float(np.sqrt(np.mean((uh - u) ** 2))))
+    for coarse, fine in zip(errs[:-1], errs[1:]):
+        assert abs(coarse / fine - 4.0) <= 0.3, errs
+
+
+def test_config4_as_given_converges():
+    """h = 1/(n+1) with folded face values (R21): not an eigenfunction, still second order."""
+    errs = []
+    for n in (16, 32, 64):
+        w = wl.config4(n)
+        uh = po.solve(w.f, w.h, w.bc)
+        errs.append(float(np.max(np.abs(uh - w.u_exact))))
+    for coarse, fine in zip(errs[:-1], errs[1:]):
+        assert abs(coarse / fine - 4.0) <= 0.3, errs
+
+
+def test_fig16_case():
+    """NN-NN-DD, omega = (1,2,3), u = cos cos sin; at 64^3 the error is the closed form."""
+    n, bc, omega = 64, (N, N, D), (1, 2, 3)
+    parts, h = mms_complex_periodic(bc, n, omega)
+    f, u = parts[0]
+    uh = po.solve(f, h, bc)
+    e = float(np.sqrt(np.mean((uh - u) ** 2)))
+    assert abs(e - closed_form_error(bc, n, omega)) <= 1e-9 * e + 1e-15
