@@ -1,0 +1,119 @@
+/*
+ * pittpack_b200 -- C ABI of the B200-native direct Poisson solver.
+ *
+ * What it computes (arxiv 1909.05423 "PittPack"; citations are lines of the paper text
+ * PAPER.md): the solution u of the second-order 7-point finite-difference Poisson equation
+ *
+ *   (u[i+1,j,k]-2u[i,j,k]+u[i-1,j,k])/dx^2 + (..j..)/dy^2 + (..k..)/dz^2 = f[i,j,k]      (eq. 3)
+ *
+ * on a directionally-uniform cell-centred nx x ny x nz grid, with one
+ * homogeneous boundary condition per axis imposed at the cell faces: periodic, Neumann
+ * (zero normal derivative) or Dirichlet (zero value, ghost cell by linear
+ * extrapolation).  Method: forward
+ * FFT / DCT-II / DST-II along x and then y chosen by each axis' boundary condition
+ * (Table 1), each built on a complex FFT with fused pre/post passes
+ * (PAPER.md:103-107); one tridiagonal Thomas solve in z per (kx,ky) with the modified-
+ * wavenumber diagonal of Table 2 -- Sherman-Morrison when z is periodic
+ * -- and the zero-mode fix; then the inverse transforms.
+ *
+ * Everything on the path is a hand-written CUDA kernel for sm_100a, fp64 throughout.  There
+ * is no cuFFT / cuSPARSE call and no CPU fallback: on a machine without a CUDA device every
+ * entry point that needs one returns PP_ERR_CUDA.
+ *
+ * Memory convention: x fastest, idx = i + nx*(j + ny*k); as a tensor, shape (nz, ny, nx),
+ * contiguous, float64.  The value at idx belongs to the cell centre ((i+1/2)dx, (j+1/2)dy,
+ * (k+1/2)dz).
+ *
+ * Singular case (all three axes periodic or Neumann): f is projected to
+ * zero mean and the zero-mean solution is returned (= the pseudo-inverse applied to f).
+ *
+ * Non-homogeneous Dirichlet face values g are the caller's job, folded into the source as
+ * PAPER.md:163 describes:  f[boundary cell] -= 2 g / h^2.
+ *
+ * Threading: a plan may be reused indefinitely, from any host thread, but concurrent
+ * pp_solve calls on ONE plan are not allowed (its tables are shared, its scratch is single).
+ * All functions return a status code; none throws, none aborts.
+ */
+#ifndef PITTPACK_B200_H
+#define PITTPACK_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pp_plan pp_plan; /* opaque; owns device tables and scratch */
+
+/* One boundary condition per axis, applied on both faces (Table 2 has matched pairs only). */
+enum { PP_BC_PERIODIC = 0, PP_BC_NEUMANN = 1, PP_BC_DIRICHLET = 2 };
+
+enum {
+    PP_SUCCESS = 0,
+    PP_ERR_INVALID_ARG = 1,      /* non-positive size/spacing, unknown BC, misaligned or partially overlapping pointers */
+    PP_ERR_UNSUPPORTED_SIZE = 2, /* nx or ny not a power of two in [4, 2048]; nz outside [2, 4096] */
+    PP_ERR_ALLOC = 3,            /* host or device allocation failed */
+    PP_ERR_CUDA = 4,             /* a CUDA runtime call or kernel launch failed (no device, bad stream, ...) */
+    PP_ERR_NULL = 5              /* a required pointer argument is NULL */
+};
+
+/* Number of kernels one pp_solve launches, and their order (for pp_plan_last_kernel_ms). */
+enum { PP_K_XFWD = 0, PP_K_YFWD = 1, PP_K_ZSOLVE = 2, PP_K_YINV = 3, PP_K_XINV = 4, PP_NUM_KERNELS = 5 };
+
+/*
+ * Create a plan for an nx x ny x nz grid with spacings dx, dy, dz and boundary conditions
+ * bc_x, bc_y, bc_z (PP_BC_*).  Mirrors the paper's construction "PoissonGPU(n0,n1,n2)" +
+ * "assignBoundary(bc)" (Listing 3).
+ *   out      : host pointer receiving the handle (set to NULL on failure).
+ *   nx, ny   : powers of two in [4, 2048] (the hand-written FFT core);  nz in [2, 4096].
+ * Synchronous.  Builds the twiddle, post-twiddle and modified-wavenumber tables on the host
+ * in extended precision and uploads them to the CURRENT device; the plan is bound to it.
+ */
+int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, double dz,
+                   int bc_x, int bc_y, int bc_z);
+
+/*
+ * Solve A u = f  (the paper's "pittPack(P)").
+ *   f, u   : DEVICE pointers to nx*ny*nz doubles, x fastest, 16-byte aligned, owned by the
+ *            caller.  u == f (exact aliasing, in place) is allowed; any other overlap is
+ *            PP_ERR_INVALID_ARG.  f is not modified unless u == f.
+ *   stream : a cudaStream_t passed as void* (NULL = the legacy default stream).
+ * Asynchronous and stream-ordered: enqueues PP_NUM_KERNELS kernels on `stream`, never
+ * allocates, never synchronises.  Launch errors are returned; execution errors surface at
+ * the caller's next synchronisation.  All passes run in place in u: no N-sized workspace.
+ */
+int pp_solve(const pp_plan *plan, const double *f, double *u, void *stream);
+
+/*
+ * Same solve with HOST buffers (nx*ny*nz doubles each; pinned memory recommended): copies
+ * f to a plan-owned device buffer, solves in place, copies the result to u_host, all on
+ * `stream`, then synchronises the stream before returning.  The device buffer is allocated
+ * on first use (PP_ERR_ALLOC if that fails) and lives until pp_plan_destroy.
+ */
+int pp_solve_host(pp_plan *plan, const double *f_host, double *u_host, void *stream);
+
+/* Free the plan and everything it owns.  NULL is a no-op returning PP_SUCCESS. */
+int pp_plan_destroy(pp_plan *plan);
+
+/* Device bytes the plan currently owns (tables + scratch + the host-solve staging buffer if created). */
+size_t pp_plan_workspace_bytes(const pp_plan *plan);
+
+/*
+ * Per-kernel timing for roofline reports.  With profiling enabled, pp_solve brackets each of
+ * its PP_NUM_KERNELS launches with CUDA events on the caller's stream (no synchronisation).
+ * pp_plan_last_kernel_ms synchronises on the last event and writes PP_NUM_KERNELS
+ * durations in milliseconds (order PP_K_*) into ms_out (host pointer).
+ */
+int pp_plan_set_profiling(pp_plan *plan, int enable);
+int pp_plan_last_kernel_ms(pp_plan *plan, float *ms_out);
+
+/* Static, NUL-terminated description of a status code. */
+const char *pp_strerror(int status);
+
+/* Library version string, e.g. "pittpack_b200 0.1 (sm_100a)". */
+const char *pp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PITTPACK_B200_H */

@@ -1,0 +1,11 @@
+"""pittpack_b200: B200-native (sm_100a, fp64) direct Poisson solver -- the single-GPU hot path of
+PittPack (arxiv 1909.05423).  The product is the C-ABI library ``libpittpack_b200.so``
+(``include/pittpack_b200.h``); this package is its thin Python binding plus the seeded workload
+generators (``workloads``).  The library is loaded on first use and there is no CPU fallback."""
+from .binding import (  # noqa: F401
+    KERNEL_NAMES, PP_BC_DIRICHLET, PP_BC_NEUMANN, PP_BC_PERIODIC, PP_NUM_KERNELS, PP_SUCCESS,
+    PittPackError, Plan, lib, pp_plan_create, pp_plan_destroy, pp_plan_last_kernel_ms,
+    pp_plan_set_profiling, pp_plan_workspace_bytes, pp_solve, pp_solve_host, strerror, version,
+)
+
+__all__ = ["Plan", "PittPackError", "lib", "version", "strerror"]

@@ -1,0 +1,195 @@
+"""Thin ctypes binding of the C ABI in include/pittpack_b200.h -- argument marshalling only;
+every step of the solve runs in the CUDA kernels of libpittpack_b200.so.
+
+The raw entry points are exported under their C names (``pp_plan_create`` ...); :class:`Plan`
+wraps them for torch tensors (torch is used for device memory and streams only).
+
+There is no CPU fallback: if the shared library is missing this module raises at first use.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+PKG_DIR = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(PKG_DIR, "libpittpack_b200.so")
+
+PP_BC_PERIODIC, PP_BC_NEUMANN, PP_BC_DIRICHLET = 0, 1, 2
+PP_SUCCESS = 0
+PP_NUM_KERNELS = 5
+KERNEL_NAMES = ("x_fwd", "y_fwd", "z_solve", "y_inv", "x_inv")
+
+EXPORTS = (
+    "pp_plan_create", "pp_solve", "pp_solve_host", "pp_plan_destroy", "pp_plan_workspace_bytes",
+    "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_strerror", "pp_version",
+)
+
+_lib = None
+
+
+class PittPackError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {strerror(status)} (status {status})")
+
+
+def lib() -> ctypes.CDLL:
+    """Load libpittpack_b200.so (once).  Fails loudly if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_1909_05423_b200.build` "
+            "(there is no CPU fallback)")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, dbl, i32 = ctypes.c_void_p, ctypes.c_double, ctypes.c_int
+    L.pp_plan_create.argtypes = [ctypes.POINTER(vp), i32, i32, i32, dbl, dbl, dbl, i32, i32, i32]
+    L.pp_plan_create.restype = i32
+    L.pp_solve.argtypes = [vp, vp, vp, vp]
+    L.pp_solve.restype = i32
+    L.pp_solve_host.argtypes = [vp, vp, vp, vp]
+    L.pp_solve_host.restype = i32
+    L.pp_plan_destroy.argtypes = [vp]
+    L.pp_plan_destroy.restype = i32
+    L.pp_plan_workspace_bytes.argtypes = [vp]
+    L.pp_plan_workspace_bytes.restype = ctypes.c_size_t
+    L.pp_plan_set_profiling.argtypes = [vp, i32]
+    L.pp_plan_set_profiling.restype = i32
+    L.pp_plan_last_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+    L.pp_plan_last_kernel_ms.restype = i32
+    L.pp_strerror.argtypes = [i32]
+    L.pp_strerror.restype = ctypes.c_char_p
+    L.pp_version.argtypes = []
+    L.pp_version.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+# ---------------------------------------------------------------- raw C-ABI calls, same names
+def pp_plan_create(nx, ny, nz, dx, dy, dz, bc_x, bc_y, bc_z):
+    """-> (status, handle).  handle is an integer address (0 on failure)."""
+    h = ctypes.c_void_p(0)
+    st = lib().pp_plan_create(ctypes.byref(h), int(nx), int(ny), int(nz), float(dx), float(dy), float(dz),
+                              int(bc_x), int(bc_y), int(bc_z))
+    return st, (h.value or 0)
+
+
+def pp_solve(plan, f_ptr, u_ptr, stream=0):
+    return lib().pp_solve(ctypes.c_void_p(plan), ctypes.c_void_p(f_ptr), ctypes.c_void_p(u_ptr),
+                          ctypes.c_void_p(stream))
+
+
+def pp_solve_host(plan, f_ptr, u_ptr, stream=0):
+    return lib().pp_solve_host(ctypes.c_void_p(plan), ctypes.c_void_p(f_ptr), ctypes.c_void_p(u_ptr),
+                               ctypes.c_void_p(stream))
+
+
+def pp_plan_destroy(plan):
+    return lib().pp_plan_destroy(ctypes.c_void_p(plan))
+
+
+def pp_plan_workspace_bytes(plan):
+    return int(lib().pp_plan_workspace_bytes(ctypes.c_void_p(plan)))
+
+
+def pp_plan_set_profiling(plan, enable):
+    return lib().pp_plan_set_profiling(ctypes.c_void_p(plan), int(bool(enable)))
+
+
+def pp_plan_last_kernel_ms(plan):
+    """-> (status, [ms] * PP_NUM_KERNELS)"""
+    buf = (ctypes.c_float * PP_NUM_KERNELS)()
+    st = lib().pp_plan_last_kernel_ms(ctypes.c_void_p(plan), buf)
+    return st, [float(v) for v in buf]
+
+
+def strerror(status: int) -> str:
+    return lib().pp_strerror(int(status)).decode()
+
+
+def version() -> str:
+    return lib().pp_version().decode()
+
+
+# ---------------------------------------------------------------- torch-facing wrapper
+_BC = {"P": PP_BC_PERIODIC, "N": PP_BC_NEUMANN, "D": PP_BC_DIRICHLET}
+
+
+def _bc_tuple(bc):
+    if isinstance(bc, str):
+        return tuple(_BC[c] for c in bc.upper())
+    return tuple(int(b) for b in bc)
+
+
+class Plan:
+    """``Plan(nx, ny, nz, dx, dy, dz, bc)`` with ``bc`` = 'PPN' or a (bc_x, bc_y, bc_z) tuple.
+
+    ``solve(f, u=None)`` takes contiguous float64 CUDA tensors of shape (nz, ny, nx) and runs on
+    torch's current stream; ``u=None`` allocates the output, ``u is f`` solves in place."""
+
+    def __init__(self, nx, ny, nz, dx, dy, dz, bc):
+        self.shape = (int(nz), int(ny), int(nx))
+        self.h = (float(dx), float(dy), float(dz))
+        self.bc = _bc_tuple(bc)
+        st, h = pp_plan_create(nx, ny, nz, dx, dy, dz, *self.bc)
+        if st != PP_SUCCESS:
+            raise PittPackError(st, "pp_plan_create")
+        self.handle = h
+
+    def _check(self, t, name):
+        import torch
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+                and tuple(t.shape) == self.shape):
+            raise ValueError(f"{name}: need a contiguous float64 CUDA tensor of shape {self.shape}")
+
+    def solve(self, f, u=None, stream=None):
+        import torch
+        self._check(f, "f")
+        if u is None:
+            u = torch.empty_like(f)
+        self._check(u, "u")
+        s = torch.cuda.current_stream(f.device) if stream is None else stream
+        st = pp_solve(self.handle, f.data_ptr(), u.data_ptr(), s.cuda_stream)
+        if st != PP_SUCCESS:
+            raise PittPackError(st, "pp_solve")
+        return u
+
+    def solve_host(self, f_host, u_host, stream=None):
+        """f_host, u_host: contiguous float64 CPU tensors (pinned recommended) of the plan's shape."""
+        import torch
+        for t, name in ((f_host, "f_host"), (u_host, "u_host")):
+            if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float64
+                    and t.is_contiguous() and tuple(t.shape) == self.shape):
+                raise ValueError(f"{name}: need a contiguous float64 CPU tensor of shape {self.shape}")
+        s = torch.cuda.current_stream() if stream is None else stream
+        st = pp_solve_host(self.handle, f_host.data_ptr(), u_host.data_ptr(), s.cuda_stream)
+        if st != PP_SUCCESS:
+            raise PittPackError(st, "pp_solve_host")
+        return u_host
+
+    def set_profiling(self, enable: bool):
+        st = pp_plan_set_profiling(self.handle, enable)
+        if st != PP_SUCCESS:
+            raise PittPackError(st, "pp_plan_set_profiling")
+
+    def last_kernel_ms(self):
+        st, ms = pp_plan_last_kernel_ms(self.handle)
+        if st != PP_SUCCESS:
+            raise PittPackError(st, "pp_plan_last_kernel_ms")
+        return dict(zip(KERNEL_NAMES, ms))
+
+    @property
+    def workspace_bytes(self):
+        return pp_plan_workspace_bytes(self.handle)
+
+    def destroy(self):
+        if getattr(self, "handle", 0):
+            pp_plan_destroy(self.handle)
+            self.handle = 0
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

@@ -1,0 +1,334 @@
+// C ABI of pittpack_b200 (include/pittpack_b200.h): plan construction, table generation and the
+// five-kernel solve.  No cuFFT / cuSPARSE, no CPU fallback.
+#include "../../include/pittpack_b200.h"
+
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "pp_fft.cuh"
+#include "pp_xpass.cuh"
+#include "pp_ypass.cuh"
+#include "pp_zsolve.cuh"
+
+using namespace pp;
+
+struct pp_plan {
+    int nx, ny, nz;
+    double dx, dy, dz;
+    int bcx, bcy, bcz;
+    int device;
+    int singular;
+    double scale;
+    double2 *tw_x, *tw_y;      // exp(-2 pi i m / n), m in [0, n)
+    double2 *ptw_x, *ptw_y;    // exp(-i pi m / (2n)), m in [0, n]
+    double *sx, *sy;           // dz^2 lam / h^2 per packed position
+    double *zero_scratch;      // [nz]
+    double *host_stage;        // N doubles, created by the first pp_solve_host
+    size_t bytes;
+    int profiling;
+    int have_times;
+    cudaEvent_t ev[PP_NUM_KERNELS + 1];
+};
+
+// ------------------------------------------------------------------------------------------
+// host-side tables, evaluated in long double and rounded once
+// ------------------------------------------------------------------------------------------
+namespace {
+
+const long double PI_L = 3.14159265358979323846264338327950288L;
+
+bool pow2_in_range(int n) { return n >= 4 && n <= 2048 && (n & (n - 1)) == 0; }
+
+void make_twiddles(int n, std::vector<double2> &tw, std::vector<double2> &ptw) {
+    tw.resize(n);
+    ptw.resize(n + 1);
+    for (int m = 0; m < n; ++m) {
+        const long double a = 2.0L * PI_L * (long double)m / (long double)n;
+        tw[m] = make_double2((double)cosl(a), (double)(-sinl(a)));
+    }
+    for (int m = 0; m <= n; ++m) {
+        const long double a = PI_L * (long double)m / (2.0L * (long double)n);
+        ptw[m] = make_double2((double)cosl(a), (double)(-sinl(a)));
+    }
+}
+
+// Table 2: modified wavenumber of wavenumber index k on an axis of length n.
+long double table2(int bc, int k, int n) {
+    long double arg;
+    if (bc == PP_BC_PERIODIC) arg = 2.0L * PI_L * (long double)k / (long double)n;
+    else if (bc == PP_BC_NEUMANN) arg = PI_L * (long double)k / (long double)n;
+    else arg = PI_L * (long double)(k + 1) / (long double)n;
+    const long double sh = sinl(0.5L * arg);
+    return -4.0L * sh * sh;                      // = -2 + 2 cos(arg), without the cancellation
+}
+
+// shift table per stored position: `packed_x` = the x-pass layout (periodic: [X_0, X_n/2, Re X_1, Im X_1, ..]),
+// otherwise position == wavenumber index (also for half-complex periodic rows: lam is even in k).
+void make_shift(int bc, int n, bool packed_x, long double factor, std::vector<double> &s) {
+    s.resize(n);
+    for (int p = 0; p < n; ++p) {
+        int k = p;
+        if (bc == PP_BC_PERIODIC && packed_x) k = (p == 0) ? 0 : ((p == 1) ? n / 2 : p / 2);
+        s[p] = (double)(factor * table2(bc, k, n));
+    }
+}
+
+template <class T>
+int upload(T **dst, const std::vector<T> &src, size_t &bytes) {
+    const size_t nb = src.size() * sizeof(T);
+    if (cudaMalloc((void **)dst, nb) != cudaSuccess) { *dst = nullptr; cudaGetLastError(); return PP_ERR_ALLOC; }
+    bytes += nb;
+    if (cudaMemcpy(*dst, src.data(), nb, cudaMemcpyHostToDevice) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    return PP_SUCCESS;
+}
+
+// ------------------------------------------------------------------------------------------
+// launch helpers
+// ------------------------------------------------------------------------------------------
+template <class K>
+int set_smem(K kernel, size_t smem) {
+    if (smem > 48 * 1024) {
+        if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+            cudaGetLastError();
+            return PP_ERR_CUDA;
+        }
+    }
+    return PP_SUCCESS;
+}
+
+template <int N>
+int launch_x(bool fwd, const double *in, double *out, long long npairs, int bc, const double2 *tw,
+             const double2 *ptw, cudaStream_t st) {
+    using X = XCfg<N>;
+    const unsigned grid = (unsigned)((npairs + X::T - 1) / X::T);
+    auto kf = xpass_fwd_kernel<N>;
+    auto ki = xpass_inv_kernel<N>;
+    if (int rc = set_smem(fwd ? kf : ki, X::SMEM)) return rc;
+    if (fwd) kf<<<grid, X::THREADS, X::SMEM, st>>>(in, out, npairs, bc, tw, ptw);
+    else     ki<<<grid, X::THREADS, X::SMEM, st>>>(in, out, npairs, bc, tw, ptw);
+    return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
+}
+
+template <int N>
+int launch_y(bool fwd, double *w, int nxh, int nz, int bc, int complex_cols, const double2 *tw,
+             const double2 *ptw, cudaStream_t st) {
+    using Y = YCfg<N>;
+    const dim3 grid((unsigned)((nxh + Y::T - 1) / Y::T), (unsigned)nz);
+    auto kf = ypass_fwd_kernel<N>;
+    auto ki = ypass_inv_kernel<N>;
+    if (int rc = set_smem(fwd ? kf : ki, Y::SMEM)) return rc;
+    if (fwd) kf<<<grid, Y::THREADS, Y::SMEM, st>>>((double2 *)w, nxh, bc, complex_cols, tw, ptw);
+    else     ki<<<grid, Y::THREADS, Y::SMEM, st>>>((double2 *)w, nxh, bc, complex_cols, tw, ptw);
+    return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
+}
+
+#define PP_DISPATCH_N(n, CALL)                       \
+    switch (n) {                                     \
+        case 4:    return CALL(4);                   \
+        case 8:    return CALL(8);                   \
+        case 16:   return CALL(16);                  \
+        case 32:   return CALL(32);                  \
+        case 64:   return CALL(64);                  \
+        case 128:  return CALL(128);                 \
+        case 256:  return CALL(256);                 \
+        case 512:  return CALL(512);                 \
+        case 1024: return CALL(1024);                \
+        case 2048: return CALL(2048);                \
+        default:   return PP_ERR_UNSUPPORTED_SIZE;   \
+    }
+
+int run_x(const pp_plan *p, bool fwd, const double *in, double *out, cudaStream_t st) {
+    const long long npairs = (long long)p->ny * p->nz / 2;
+#define CALL_X(NN) launch_x<NN>(fwd, in, out, npairs, p->bcx, p->tw_x, p->ptw_x, st)
+    PP_DISPATCH_N(p->nx, CALL_X)
+#undef CALL_X
+}
+
+int run_y(const pp_plan *p, bool fwd, double *w, cudaStream_t st) {
+    const int complex_cols = (p->bcx == PP_BC_PERIODIC && p->bcy == PP_BC_PERIODIC) ? 1 : 0;
+#define CALL_Y(NN) launch_y<NN>(fwd, w, p->nx / 2, p->nz, p->bcy, complex_cols, p->tw_y, p->ptw_y, st)
+    PP_DISPATCH_N(p->ny, CALL_Y)
+#undef CALL_Y
+}
+
+int run_z(const pp_plan *p, double *w, cudaStream_t st) {
+    ZParams zp;
+    zp.nx = p->nx; zp.ny = p->ny; zp.nz = p->nz;
+    zp.bcz = p->bcz;
+    zp.singular = p->singular;
+    zp.scale = p->scale;
+    zp.sx = p->sx; zp.sy = p->sy;
+    zp.zero_scratch = p->zero_scratch;
+    const size_t plane = (size_t)p->nx * p->ny;
+    const unsigned grid = (unsigned)((plane + 255) / 256);
+    const int cb = (p->nz <= 16 * Z_MAX_CK) ? 16 : ((p->nz <= 32 * Z_MAX_CK) ? 32 : 64);
+    if (p->bcz == PP_BC_PERIODIC) {
+        if (cb == 16)      zsolve_cyclic_kernel<16><<<grid, 256, 0, st>>>(w, zp);
+        else if (cb == 32) zsolve_cyclic_kernel<32><<<grid, 256, 0, st>>>(w, zp);
+        else               zsolve_cyclic_kernel<64><<<grid, 256, 0, st>>>(w, zp);
+    } else {
+        if (cb == 16)      zsolve_thomas_kernel<16><<<grid, 256, 0, st>>>(w, zp);
+        else if (cb == 32) zsolve_thomas_kernel<32><<<grid, 256, 0, st>>>(w, zp);
+        else               zsolve_thomas_kernel<64><<<grid, 256, 0, st>>>(w, zp);
+    }
+    return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
+}
+
+void free_plan(pp_plan *p) {
+    if (!p) return;
+    cudaFree(p->tw_x); cudaFree(p->tw_y); cudaFree(p->ptw_x); cudaFree(p->ptw_y);
+    cudaFree(p->sx); cudaFree(p->sy); cudaFree(p->zero_scratch); cudaFree(p->host_stage);
+    for (auto &e : p->ev) if (e) cudaEventDestroy(e);
+    cudaGetLastError();
+    delete p;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// C ABI
+// ------------------------------------------------------------------------------------------
+extern "C" {
+
+const char *pp_version(void) { return "pittpack_b200 0.1 (sm_100a)"; }
+
+const char *pp_strerror(int status) {
+    switch (status) {
+        case PP_SUCCESS: return "success";
+        case PP_ERR_INVALID_ARG: return "invalid argument";
+        case PP_ERR_UNSUPPORTED_SIZE: return "unsupported grid size (nx, ny: powers of two in [4, 2048]; nz in [2, 4096])";
+        case PP_ERR_ALLOC: return "allocation failed";
+        case PP_ERR_CUDA: return "CUDA runtime or launch error (is a CUDA device present?)";
+        case PP_ERR_NULL: return "null pointer argument";
+        default: return "unknown status";
+    }
+}
+
+int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, double dz,
+                   int bc_x, int bc_y, int bc_z) {
+    if (!out) return PP_ERR_NULL;
+    *out = nullptr;
+    if (nx <= 0 || ny <= 0 || nz <= 0) return PP_ERR_INVALID_ARG;
+    if (!(dx > 0.0) || !(dy > 0.0) || !(dz > 0.0) || !std::isfinite(dx) || !std::isfinite(dy) || !std::isfinite(dz))
+        return PP_ERR_INVALID_ARG;
+    for (int bc : {bc_x, bc_y, bc_z})
+        if (bc != PP_BC_PERIODIC && bc != PP_BC_NEUMANN && bc != PP_BC_DIRICHLET) return PP_ERR_INVALID_ARG;
+    if (!pow2_in_range(nx) || !pow2_in_range(ny) || nz < 2 || nz > 64 * Z_MAX_CK) return PP_ERR_UNSUPPORTED_SIZE;
+
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+
+    pp_plan *p = new (std::nothrow) pp_plan();
+    if (!p) return PP_ERR_ALLOC;
+    std::memset(p, 0, sizeof(*p));
+    p->nx = nx; p->ny = ny; p->nz = nz;
+    p->dx = dx; p->dy = dy; p->dz = dz;
+    p->bcx = bc_x; p->bcy = bc_y; p->bcz = bc_z;
+    p->device = dev;
+    p->singular = (bc_x != PP_BC_DIRICHLET && bc_y != PP_BC_DIRICHLET && bc_z != PP_BC_DIRICHLET) ? 1 : 0;
+    p->scale = (double)((long double)dz * (long double)dz / ((long double)nx * (long double)ny));
+
+    std::vector<double2> tw, ptw;
+    std::vector<double> s;
+    int rc = PP_SUCCESS;
+    make_twiddles(nx, tw, ptw);
+    if (!rc) rc = upload(&p->tw_x, tw, p->bytes);
+    if (!rc) rc = upload(&p->ptw_x, ptw, p->bytes);
+    make_twiddles(ny, tw, ptw);
+    if (!rc) rc = upload(&p->tw_y, tw, p->bytes);
+    if (!rc) rc = upload(&p->ptw_y, ptw, p->bytes);
+    const long double dz2 = (long double)dz * (long double)dz;
+    make_shift(bc_x, nx, true, dz2 / ((long double)dx * (long double)dx), s);
+    if (!rc) rc = upload(&p->sx, s, p->bytes);
+    make_shift(bc_y, ny, false, dz2 / ((long double)dy * (long double)dy), s);
+    if (!rc) rc = upload(&p->sy, s, p->bytes);
+    if (!rc) {
+        std::vector<double> z((size_t)nz, 0.0);
+        rc = upload(&p->zero_scratch, z, p->bytes);
+    }
+    if (!rc) {
+        for (auto &e : p->ev)
+            if (cudaEventCreate(&e) != cudaSuccess) { e = nullptr; cudaGetLastError(); rc = PP_ERR_CUDA; break; }
+    }
+    if (rc) { free_plan(p); return rc; }
+    *out = p;
+    return PP_SUCCESS;
+}
+
+int pp_solve(const pp_plan *plan, const double *f, double *u, void *stream) {
+    if (!plan || !f || !u) return PP_ERR_NULL;
+    const size_t n = (size_t)plan->nx * plan->ny * plan->nz;
+    if (((uintptr_t)f & 15) || ((uintptr_t)u & 15)) return PP_ERR_INVALID_ARG;
+    if (f != u) {
+        const uintptr_t a = (uintptr_t)f, b = (uintptr_t)u, len = n * sizeof(double);
+        if (a < b + len && b < a + len) return PP_ERR_INVALID_ARG;     // partial overlap
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    pp_plan *mp = const_cast<pp_plan *>(plan);
+    const bool prof = plan->profiling != 0;
+    int rc;
+#define PP_MARK(i) if (prof && cudaEventRecord(mp->ev[i], st) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    PP_MARK(0)
+    if ((rc = run_x(plan, true, f, u, st))) return rc;          // a1-a3: x pre / FFT / post
+    PP_MARK(1)
+    if ((rc = run_y(plan, true, u, st))) return rc;             // a4-a6: y pre / FFT / post
+    PP_MARK(2)
+    if ((rc = run_z(plan, u, st))) return rc;                   // a7-a8: diagonal + tridiagonal solve
+    PP_MARK(3)
+    if ((rc = run_y(plan, false, u, st))) return rc;            // a9: y inverse
+    PP_MARK(4)
+    if ((rc = run_x(plan, false, u, u, st))) return rc;         // a10: x inverse
+    PP_MARK(5)
+#undef PP_MARK
+    if (prof) mp->have_times = 1;
+    return PP_SUCCESS;
+}
+
+int pp_solve_host(pp_plan *plan, const double *f_host, double *u_host, void *stream) {
+    if (!plan || !f_host || !u_host) return PP_ERR_NULL;
+    const size_t nb = (size_t)plan->nx * plan->ny * plan->nz * sizeof(double);
+    if (!plan->host_stage) {
+        if (cudaMalloc((void **)&plan->host_stage, nb) != cudaSuccess) {
+            plan->host_stage = nullptr;
+            cudaGetLastError();
+            return PP_ERR_ALLOC;
+        }
+        plan->bytes += nb;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    if (cudaMemcpyAsync(plan->host_stage, f_host, nb, cudaMemcpyHostToDevice, st) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    if (int rc = pp_solve(plan, plan->host_stage, plan->host_stage, stream)) return rc;
+    if (cudaMemcpyAsync(u_host, plan->host_stage, nb, cudaMemcpyDeviceToHost, st) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    if (cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    return PP_SUCCESS;
+}
+
+int pp_plan_destroy(pp_plan *plan) {
+    free_plan(plan);
+    return PP_SUCCESS;
+}
+
+size_t pp_plan_workspace_bytes(const pp_plan *plan) { return plan ? plan->bytes : 0; }
+
+int pp_plan_set_profiling(pp_plan *plan, int enable) {
+    if (!plan) return PP_ERR_NULL;
+    plan->profiling = enable ? 1 : 0;
+    plan->have_times = 0;
+    return PP_SUCCESS;
+}
+
+int pp_plan_last_kernel_ms(pp_plan *plan, float *ms_out) {
+    if (!plan || !ms_out) return PP_ERR_NULL;
+    if (!plan->have_times) return PP_ERR_INVALID_ARG;
+    if (cudaEventSynchronize(plan->ev[PP_NUM_KERNELS]) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    for (int i = 0; i < PP_NUM_KERNELS; ++i)
+        if (cudaEventElapsedTime(&ms_out[i], plan->ev[i], plan->ev[i + 1]) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    return PP_SUCCESS;
+}
+
+}  // extern "C"

@@ -1,0 +1,215 @@
+// x-pass kernels: the transform along the contiguous x axis, forward (first pass of the solve)
+// and inverse (last pass), with the boundary-condition pre/post-processing fused in
+// ("pre-processing / complex FFT / post-processing").
+//
+// Two real rows (2p, 2p+1 of the ny*nz rows) ride one complex FFT, z = a + i b; the Hermitian
+// symmetry of a real signal's spectrum ("Enforce Hermitian symmetry") separates
+// them afterwards:  A_m = (Z_m + conj Z_{N-m})/2,  B_m = (Z_m - conj Z_{N-m})/(2i).
+//
+//   periodic  (eq. 6)   packed half spectrum in N doubles per row:
+//             [Re X_0, Re X_{N/2}, Re X_1, Im X_1, ..., Re X_{N/2-1}, Im X_{N/2-1}]
+//   Neumann   (eq. 7, DCT-II)         Makhoul: v_i = z_{2i}, v_{N-1-i} = z_{2i+1},
+//             Y_m = Re(w^m V_m), Y_{N-m} = -Im(w^m V_m), w = exp(-i pi/2N)
+//   Dirichlet (eq. 9, DST-II)         the same around the wrapper [u5,-u4,u3,-u2,u1] on input and
+//             output
+// Inverse transforms (eq. 8 / eq. 10): V_m = conj(w)^m (Y_m - i Y_{N-m}),
+// Y_N = 0, inverse FFT, un-permute.  All unnormalised; 1/(nx ny) is applied in the z solve.
+#pragma once
+#include "pp_fft.cuh"
+
+namespace pp {
+
+constexpr int BC_P = 0, BC_N = 1, BC_D = 2;
+
+struct LayoutLin {
+    __device__ __forceinline__ int operator()(int i) const { return pad8(i); }
+};
+
+// synchronise the P threads of one transform inside a CTA of T transforms
+template <int P, int T>
+struct GroupSync {
+    int id;   // transform index within the CTA
+    __device__ __forceinline__ void operator()() const {
+        if constexpr (P >= 64 && T > 1 && T <= 15) {
+            asm volatile("bar.sync %0, %1;" ::"r"(id + 1), "n"(P) : "memory");
+        } else if constexpr (P <= 32 && (P * T) % 32 == 0) {
+            __syncwarp();
+        } else {
+            __syncthreads();
+        }
+    }
+};
+
+__device__ __forceinline__ double sgn_of(int i) { return (i & 1) ? -1.0 : 1.0; }
+
+template <int N>
+struct XCfg {
+    static constexpr int P = FftCfg<N>::P;
+    static constexpr int T = (256 / P) > 0 ? (256 / P) : 1;   // transforms (row pairs) per CTA; <= 4 when P >= 64
+    static constexpr int THREADS = T * P;
+    static constexpr size_t SMEM = size_t(T) * FftCfg<N>::SMEM_ELEMS * sizeof(double2);
+};
+
+// ------------------------------------------------------------------------------------------
+// forward: real rows -> spectral rows
+// ------------------------------------------------------------------------------------------
+template <int N>
+__global__ void __launch_bounds__(XCfg<N>::THREADS)
+xpass_fwd_kernel(const double *in, double *out, long long npairs, int bc,
+                 const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
+    using C = FftCfg<N>;
+    constexpr int E = C::E, P = C::P, T = XCfg<N>::T, H = N / 2;
+    extern __shared__ double2 smem[];
+    const int f = threadIdx.x / P, t = threadIdx.x % P;
+    const long long pair = (long long)blockIdx.x * T + f;
+    const bool active = pair < npairs;
+    const long long row = active ? pair * 2 : 0;
+    const double *ra = in + row * N, *rb = ra + N;
+    double *oa = out + row * N, *ob = oa + N;
+    double2 *s = smem + f * C::SMEM_ELEMS;
+    const LayoutLin lay;
+    const GroupSync<P, T> sync{f};
+
+    // ---- pre-processing fused into the load
+    double2 v[E];
+#pragma unroll
+    for (int q = 0; q < E; ++q) {
+        const int i = t + q * P;
+        if (bc == BC_P) {
+            v[q] = make_double2(ra[i], rb[i]);
+        } else if (bc == BC_N) {
+            const int p = (i < H) ? 2 * i : 2 * (N - 1 - i) + 1;
+            v[q] = make_double2(ra[p], rb[p]);
+        } else {
+            // z'_m = (-1)^m z_{N-1-m}, then the Makhoul permutation
+            if (i < H) { const int p = N - 1 - 2 * i; v[q] = make_double2(ra[p], rb[p]); }
+            else       { const int p = 2 * i - N;     v[q] = make_double2(-ra[p], -rb[p]); }
+        }
+    }
+
+    fft<N, FWD>(v, t, s, tw, lay, sync);
+
+    // ---- post-processing: Hermitian separation of the two rows, twiddle, store
+#pragma unroll
+    for (int q = 0; q < E; ++q) s[lay(t + q * P)] = v[q];
+    sync();
+    if (active) {
+#pragma unroll
+        for (int q = 0; q < E / 2; ++q) {
+            const int m = t + q * P;                       // 0 <= m < N/2
+            const double2 zm = v[q];
+            const double2 zc = s[lay((N - m) & (N - 1))];
+            if (m == 0) {
+                const double2 zh = v[E / 2];               // thread 0 also holds Z_{N/2}
+                if (bc == BC_P) {
+                    *reinterpret_cast<double2 *>(oa) = make_double2(zm.x, zh.x);
+                    *reinterpret_cast<double2 *>(ob) = make_double2(zm.y, zh.y);
+                } else {
+                    const double c4 = ptw[H].x;            // cos(pi/4)
+                    if (bc == BC_N) {
+                        oa[0] = zm.x; ob[0] = zm.y;
+                        oa[H] = c4 * zh.x; ob[H] = c4 * zh.y;
+                    } else {                               // logical m -> N-1-m, sign -(-1)^m
+                        oa[N - 1] = -zm.x; ob[N - 1] = -zm.y;
+                        const double sg = -sgn_of(H);
+                        oa[N - 1 - H] = sg * c4 * zh.x; ob[N - 1 - H] = sg * c4 * zh.y;
+                    }
+                }
+            } else {
+                const double2 A = make_double2(0.5 * (zm.x + zc.x), 0.5 * (zm.y - zc.y));
+                const double2 B = make_double2(0.5 * (zm.y + zc.y), -0.5 * (zm.x - zc.x));
+                if (bc == BC_P) {
+                    *reinterpret_cast<double2 *>(oa + 2 * m) = A;
+                    *reinterpret_cast<double2 *>(ob + 2 * m) = B;
+                } else {
+                    const double2 w = __ldg(&ptw[m]);
+                    const double2 ca = cmul(w, A), cb = cmul(w, B);
+                    if (bc == BC_N) {
+                        oa[m] = ca.x;      ob[m] = cb.x;
+                        oa[N - m] = -ca.y; ob[N - m] = -cb.y;
+                    } else {
+                        const double s1 = -sgn_of(m);                  // for logical m
+                        oa[N - 1 - m] = s1 * ca.x; ob[N - 1 - m] = s1 * cb.x;
+                        // logical N-m -> position m-1, sign -(-1)^(N-m) = -(-1)^m
+                        oa[m - 1] = -s1 * ca.y;    ob[m - 1] = -s1 * cb.y;
+                    }
+                }
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// inverse: spectral rows -> real rows
+// ------------------------------------------------------------------------------------------
+template <int N>
+__global__ void __launch_bounds__(XCfg<N>::THREADS)
+xpass_inv_kernel(const double *in, double *out, long long npairs, int bc,
+                 const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
+    using C = FftCfg<N>;
+    constexpr int E = C::E, P = C::P, T = XCfg<N>::T, H = N / 2;
+    extern __shared__ double2 smem[];
+    const int f = threadIdx.x / P, t = threadIdx.x % P;
+    const long long pair = (long long)blockIdx.x * T + f;
+    const bool active = pair < npairs;
+    const long long row = active ? pair * 2 : 0;
+    const double *ra = in + row * N, *rb = ra + N;
+    double *oa = out + row * N, *ob = oa + N;
+    double2 *s = smem + f * C::SMEM_ELEMS;
+    const LayoutLin lay;
+    const GroupSync<P, T> sync{f};
+
+    double2 v[E];
+#pragma unroll
+    for (int q = 0; q < E; ++q) {
+        const int m = t + q * P;
+        if (bc == BC_P) {
+            double2 A, B;
+            if (m == 0)      { A = make_double2(ra[0], 0.0); B = make_double2(rb[0], 0.0); }
+            else if (m == H) { A = make_double2(ra[1], 0.0); B = make_double2(rb[1], 0.0); }
+            else if (m < H)  { A = *reinterpret_cast<const double2 *>(ra + 2 * m);
+                               B = *reinterpret_cast<const double2 *>(rb + 2 * m); }
+            else             { A = cconj(*reinterpret_cast<const double2 *>(ra + 2 * (N - m)));
+                               B = cconj(*reinterpret_cast<const double2 *>(rb + 2 * (N - m))); }
+            v[q] = make_double2(A.x - B.y, A.y + B.x);                 // Z = A + i B
+        } else {
+            double ya, yb, yap, ybp;
+            if (bc == BC_N) {
+                ya = ra[m]; yb = rb[m];
+                yap = (m == 0) ? 0.0 : ra[N - m];
+                ybp = (m == 0) ? 0.0 : rb[N - m];
+            } else {                                                   // Y'_m = (-1)^m S_{N-1-m}
+                const double s1 = sgn_of(m);
+                ya = s1 * ra[N - 1 - m]; yb = s1 * rb[N - 1 - m];
+                yap = (m == 0) ? 0.0 : s1 * ra[m - 1];                 // (-1)^(N-m) S_{m-1}
+                ybp = (m == 0) ? 0.0 : s1 * rb[m - 1];
+            }
+            const double2 w = cconj(__ldg(&ptw[m]));
+            v[q] = cmul(w, make_double2(ya + ybp, yb - yap));          // conj(w)^m (Y_m - i Y_{N-m})
+        }
+    }
+    // all loads of this row pair are done before any thread of the group stores (in-place safe):
+    // the FFT's exchanges synchronise the group; for single-stage transforms sync explicitly
+    if constexpr (C::R0 == N) sync();
+
+    fft<N, INV>(v, t, s, tw, lay, sync);
+
+    if (active) {
+#pragma unroll
+        for (int q = 0; q < E; ++q) {
+            const int i = t + q * P;
+            if (bc == BC_P) {
+                oa[i] = v[q].x; ob[i] = v[q].y;
+            } else {
+                const int p = (i < H) ? 2 * i : 2 * (N - 1 - i) + 1;   // un-permute
+                if (bc == BC_N) { oa[p] = v[q].x; ob[p] = v[q].y; }
+                else {                                                 // x_{N-1-p} = -(-1)^p x'_p
+                    const double s1 = -sgn_of(p);
+                    oa[N - 1 - p] = s1 * v[q].x; ob[N - 1 - p] = s1 * v[q].y;
+                }
+            }
+        }
+    }
+}
+
+}  // namespace pp

@@ -1,0 +1,202 @@
+// y-pass kernels: the transform along y (stride = one x row), forward and inverse, in place.
+//
+// On one GPU the paper's chunk exchange + data shuffle before the y transform (PAPER.md:386-403,
+// Fig. 13) becomes an in-HBM tiled transpose: a CTA owns T adjacent double2 columns (T*16 bytes
+// contiguous per row) for all ny rows of one z plane, pulls them into registers with coalesced
+// row-segment loads, runs the shared-memory FFT core down each column, and writes the tile back.
+//
+// The x-pass left every row as nx/2 double2 elements.  A double2 column is either
+//   * a complex column  -- x periodic, column >= 1: (Re, Im) of one kx mode.  With y periodic it
+//     gets a plain complex FFT (eq. 6); or
+//   * a pair of independent real columns (x Neumann/Dirichlet; or column 0 of periodic x, which
+//     holds the real kx = 0 and kx = nx/2 modes; or any column when y is Neumann/Dirichlet, whose
+//     real transforms act on Re and Im separately).  The pair rides one complex FFT and is
+//     separated by Hermitian symmetry exactly as in the x-pass.
+// Row layout after the forward pass:
+//   y periodic, complex column:  row m = Z_m
+//   y periodic, real pair:       "half-complex" rows: row 0 = (A_0, B_0), row N/2 = (A_N/2, B_N/2),
+//                                row m = (Re A_m, Re B_m), row N-m = (Im A_m, Im B_m), 0 < m < N/2
+//   y Neumann / Dirichlet:       row m = (Ya_m, Yb_m)  (DCT-II / DST-II coefficients, eq. 7 / 9)
+// In every case the modified wavenumber of row m is Table 2's evaluated at m,
+// because the periodic eigenvalue is even in m -- so the z solve needs one table per axis.
+#pragma once
+#include "pp_xpass.cuh"
+
+namespace pp {
+
+template <int T>
+struct LayoutCol {
+    int c;
+    __device__ __forceinline__ int operator()(int i) const { return pad8(i) * T + c; }
+};
+
+struct SyncCta {
+    __device__ __forceinline__ void operator()() const { __syncthreads(); }
+};
+
+template <int N>
+struct YCfg {
+    static constexpr int P = FftCfg<N>::P;
+    static constexpr int T = (N <= 512) ? 8 : 4;        // double2 columns per CTA (128 / 64 B row segments)
+    static constexpr int THREADS = T * P;
+    static constexpr size_t SMEM = size_t(T) * FftCfg<N>::SMEM_ELEMS * sizeof(double2);
+};
+
+__device__ __forceinline__ double2 dscale(double a, double2 v) { return make_double2(a * v.x, a * v.y); }
+
+template <int N>
+__global__ void __launch_bounds__(YCfg<N>::THREADS)
+ypass_fwd_kernel(double2 *w, int nxh, int bc, int complex_cols,
+                 const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
+    using C = FftCfg<N>;
+    constexpr int E = C::E, P = C::P, T = YCfg<N>::T, H = N / 2;
+    extern __shared__ double2 smem[];
+    const int c = threadIdx.x % T, t = threadIdx.x / T;
+    const int cp = blockIdx.x * T + c;
+    const bool active = cp < nxh;
+    double2 *base = w + (size_t)blockIdx.y * N * nxh + (active ? cp : 0);
+    const size_t ld = nxh;
+    const LayoutCol<T> lay{c};
+    const SyncCta sync;
+
+    double2 v[E];
+#pragma unroll
+    for (int q = 0; q < E; ++q) {
+        const int i = t + q * P;
+        if (bc == BC_P) {
+            v[q] = base[i * ld];
+        } else if (bc == BC_N) {
+            const int p = (i < H) ? 2 * i : 2 * (N - 1 - i) + 1;
+            v[q] = base[p * ld];
+        } else {
+            if (i < H) v[q] = base[(N - 1 - 2 * i) * ld];
+            else       v[q] = dscale(-1.0, base[(2 * i - N) * ld]);
+        }
+    }
+
+    fft<N, FWD>(v, t, smem, tw, lay, sync);
+
+    if (complex_cols && blockIdx.x > 0) {                  // block-uniform: all columns complex
+        if (active) {
+#pragma unroll
+            for (int q = 0; q < E; ++q) base[(t + q * P) * ld] = v[q];
+        }
+        return;
+    }
+#pragma unroll
+    for (int q = 0; q < E; ++q) smem[lay(t + q * P)] = v[q];
+    __syncthreads();
+    if (!active) return;
+    if (complex_cols && cp > 0) {
+#pragma unroll
+        for (int q = 0; q < E; ++q) base[(t + q * P) * ld] = v[q];
+        return;
+    }
+#pragma unroll
+    for (int q = 0; q < E / 2; ++q) {
+        const int m = t + q * P;
+        const double2 zm = v[q];
+        const double2 zc = smem[lay((N - m) & (N - 1))];
+        if (m == 0) {
+            const double2 zh = v[E / 2];
+            if (bc == BC_P) {
+                base[0] = zm;
+                base[H * ld] = zh;
+            } else {
+                const double c4 = ptw[H].x;
+                if (bc == BC_N) {
+                    base[0] = zm;
+                    base[H * ld] = dscale(c4, zh);
+                } else {
+                    base[(N - 1) * ld] = dscale(-1.0, zm);
+                    base[(N - 1 - H) * ld] = dscale(-sgn_of(H) * c4, zh);
+                }
+            }
+        } else {
+            const double2 A = make_double2(0.5 * (zm.x + zc.x), 0.5 * (zm.y - zc.y));
+            const double2 B = make_double2(0.5 * (zm.y + zc.y), -0.5 * (zm.x - zc.x));
+            if (bc == BC_P) {
+                base[m * ld] = make_double2(A.x, B.x);
+                base[(N - m) * ld] = make_double2(A.y, B.y);
+            } else {
+                const double2 wm = __ldg(&ptw[m]);
+                const double2 ca = cmul(wm, A), cb = cmul(wm, B);
+                if (bc == BC_N) {
+                    base[m * ld] = make_double2(ca.x, cb.x);
+                    base[(N - m) * ld] = make_double2(-ca.y, -cb.y);
+                } else {
+                    const double s1 = -sgn_of(m);
+                    base[(N - 1 - m) * ld] = make_double2(s1 * ca.x, s1 * cb.x);
+                    base[(m - 1) * ld] = make_double2(-s1 * ca.y, -s1 * cb.y);
+                }
+            }
+        }
+    }
+}
+
+template <int N>
+__global__ void __launch_bounds__(YCfg<N>::THREADS)
+ypass_inv_kernel(double2 *w, int nxh, int bc, int complex_cols,
+                 const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
+    using C = FftCfg<N>;
+    constexpr int E = C::E, P = C::P, T = YCfg<N>::T, H = N / 2;
+    extern __shared__ double2 smem[];
+    const int c = threadIdx.x % T, t = threadIdx.x / T;
+    const int cp = blockIdx.x * T + c;
+    const bool active = cp < nxh;
+    double2 *base = w + (size_t)blockIdx.y * N * nxh + (active ? cp : 0);
+    const size_t ld = nxh;
+    const LayoutCol<T> lay{c};
+    const SyncCta sync;
+    const bool cplx = complex_cols && cp > 0;
+
+    double2 v[E];
+#pragma unroll
+    for (int q = 0; q < E; ++q) {
+        const int m = t + q * P;
+        if (cplx) {
+            v[q] = base[m * ld];
+        } else if (bc == BC_P) {
+            if (m == 0 || m == H) {
+                v[q] = base[m * ld];                                   // (A, B) both real: Z = A + i B
+            } else if (m < H) {
+                const double2 lo = base[m * ld], hi = base[(N - m) * ld];
+                v[q] = make_double2(lo.x - hi.y, hi.x + lo.y);
+            } else {
+                const double2 lo = base[(N - m) * ld], hi = base[m * ld];
+                v[q] = make_double2(lo.x + hi.y, lo.y - hi.x);
+            }
+        } else {
+            double2 ym, yp;
+            if (bc == BC_N) {
+                ym = base[m * ld];
+                yp = (m == 0) ? make_double2(0.0, 0.0) : base[(N - m) * ld];
+            } else {
+                const double s1 = sgn_of(m);
+                ym = dscale(s1, base[(N - 1 - m) * ld]);
+                yp = (m == 0) ? make_double2(0.0, 0.0) : dscale(s1, base[(m - 1) * ld]);
+            }
+            const double2 wm = cconj(__ldg(&ptw[m]));
+            v[q] = cmul(wm, make_double2(ym.x + yp.y, ym.y - yp.x));
+        }
+    }
+    // in place: every load of the tile precedes every store -- the FFT's exchanges are CTA-wide
+    // barriers; a single-stage transform has P = 1 (one thread owns the whole column)
+
+    fft<N, INV>(v, t, smem, tw, lay, sync);
+
+    if (!active) return;
+#pragma unroll
+    for (int q = 0; q < E; ++q) {
+        const int i = t + q * P;
+        if (bc == BC_P) {
+            base[i * ld] = v[q];
+        } else {
+            const int p = (i < H) ? 2 * i : 2 * (N - 1 - i) + 1;
+            if (bc == BC_N) base[p * ld] = v[q];
+            else            base[(N - 1 - p) * ld] = dscale(-sgn_of(p), v[q]);
+        }
+    }
+}
+
+}  // namespace pp

@@ -1,0 +1,109 @@
+"""GPU tests of the C-ABI contract: aliasing, plan reuse, determinism, streams, host solve,
+error codes, profiling hooks."""
+import ctypes
+
+import numpy as np
+import pytest
+
+from oracle import poisson_oracle as po
+from paper_1909_05423_b200 import workloads as wl
+from gpu_util import TOL, gpu_solve, rel_err
+
+pytestmark = pytest.mark.gpu
+
+
+def test_in_place_equals_out_of_place_and_f_untouched():
+    import torch
+    import paper_1909_05423_b200 as pp
+    w = wl.config2("PPN", "normal", n=64)
+    plan = pp.Plan(64, 64, 64, *w.h, w.bc)
+    f = torch.from_numpy(w.f).cuda()
+    f0 = f.clone()
+    u = plan.solve(f)
+    torch.cuda.synchronize()
+    assert torch.equal(f, f0)
+    g = f.clone()
+    plan.solve(g, g)
+    torch.cuda.synchronize()
+    assert torch.equal(g, u)                      # bitwise: same kernels, same order
+    assert rel_err(u.cpu().numpy(), po.solve(w.f, w.h, w.bc)) <= TOL
+    plan.destroy()
+
+
+def test_plan_reuse_and_determinism():
+    import torch
+    import paper_1909_05423_b200 as pp
+    w = wl.config2("NND", "normal", n=64)
+    plan = pp.Plan(64, 64, 64, *w.h, w.bc)
+    f = torch.from_numpy(w.f).cuda()
+    outs = [plan.solve(f).clone() for _ in range(4)]
+    torch.cuda.synchronize()
+    for o in outs[1:]:
+        assert torch.equal(o, outs[0])
+    f2 = torch.from_numpy(wl.random_uniform(w.shape, 5)).cuda()
+    u2 = plan.solve(f2)
+    assert rel_err(u2.cpu().numpy(), po.solve(f2.cpu().numpy(), w.h, w.bc)) <= TOL
+    plan.destroy()
+
+
+def test_non_default_stream_is_ordered():
+    import torch
+    import paper_1909_05423_b200 as pp
+    w = wl.config1("uniform")
+    plan = pp.Plan(32, 32, 32, *w.h, w.bc)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        f = torch.from_numpy(w.f).cuda(non_blocking=False)
+        f.mul_(2.0)                                # queued on s before the solve
+        u = plan.solve(f)
+        u.mul_(0.5)                                # queued on s after the solve
+    s.synchronize()
+    assert rel_err(u.cpu().numpy(), po.solve(w.f, w.h, w.bc)) <= TOL
+    plan.destroy()
+
+
+def test_host_solve():
+    import torch
+    import paper_1909_05423_b200 as pp
+    w = wl.config2("PPD", "normal", n=32)
+    plan = pp.Plan(32, 32, 32, *w.h, w.bc)
+    before = plan.workspace_bytes
+    fh = torch.from_numpy(w.f).pin_memory()
+    uh = torch.empty_like(fh).pin_memory()
+    plan.solve_host(fh, uh)
+    assert plan.workspace_bytes == before + w.f.nbytes
+    assert rel_err(uh.numpy(), po.solve(w.f, w.h, w.bc)) <= TOL
+    plan.destroy()
+
+
+def test_profiling_hooks():
+    import torch
+    import paper_1909_05423_b200 as pp
+    w = wl.config1("uniform")
+    plan = pp.Plan(32, 32, 32, *w.h, w.bc)
+    f = torch.from_numpy(w.f).cuda()
+    with pytest.raises(pp.PittPackError):
+        plan.last_kernel_ms()                     # nothing recorded yet
+    plan.set_profiling(True)
+    plan.solve(f)
+    ms = plan.last_kernel_ms()
+    assert list(ms) == list(pp.KERNEL_NAMES) and all(v > 0 for v in ms.values())
+    plan.destroy()
+
+
+def test_error_codes_on_device():
+    import torch
+    import paper_1909_05423_b200 as pp
+    st, h = pp.pp_plan_create(32, 32, 32, 0.1, 0.1, 0.1, 0, 0, 2)
+    assert st == 0 and h
+    f = torch.zeros(32 * 32 * 32 + 8, dtype=torch.float64, device="cuda")
+    n = 32 * 32 * 32
+    assert pp.pp_solve(h, 0, f.data_ptr()) == 5                               # NULL
+    assert pp.pp_solve(0, f.data_ptr(), f.data_ptr()) == 5
+    assert pp.pp_solve(h, f.data_ptr() + 8, f.data_ptr() + 8) == 1            # misaligned
+    assert pp.pp_solve(h, f.data_ptr(), f.data_ptr() + 64) == 1               # partial overlap
+    assert pp.pp_solve(h, f.data_ptr(), f.data_ptr()) == 0                    # exact alias is fine
+    torch.cuda.synchronize()
+    assert pp.pp_plan_destroy(h) == 0
+    assert pp.pp_plan_destroy(0) == 0
+    del n

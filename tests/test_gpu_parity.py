@@ -1,0 +1,107 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, element by element, on the
+same seeded inputs.  Bar: max|u_gpu - u_ref| / max|u_ref| <= 1e-11 (north_star)."""
+import itertools
+
+import numpy as np
+import pytest
+
+from oracle import poisson_oracle as po
+from paper_1909_05423_b200 import workloads as wl
+from gpu_util import TOL, gpu_solve, rel_err
+
+pytestmark = pytest.mark.gpu
+
+ALL27 = ["".join(c) for c in itertools.product("PND", repeat=3)]
+
+
+def check(w: wl.Workload, tol=TOL, **kw):
+    u = gpu_solve(w.f, w.h, w.bc, **kw)
+    ref = po.solve(w.f, w.h, w.bc)
+    e = rel_err(u, ref)
+    assert e <= tol, (w.name, e)
+    return u, ref
+
+
+@pytest.mark.parametrize("combo", ALL27)
+@pytest.mark.parametrize("shape", [(12, 8, 16), (5, 32, 8), (40, 16, 64)], ids=lambda s: "x".join(map(str, s[::-1])))
+def test_all_27_combos_small(combo, shape):
+    """Every boundary-condition combination; non-cubic, nz not a power of two, anisotropic spacing."""
+    bc = wl.parse_bc(combo)
+    nz, ny, nx = shape
+    h = (1.0 / nx, 0.7 / ny, 1.3 / nz)
+    f = wl.random_uniform(shape, 7 + ALL27.index(combo))
+    check(wl.Workload(f"{combo}-{shape}", shape, h, bc, f))
+
+
+@pytest.mark.parametrize("n", [4, 8, 16, 32, 64, 128, 256, 512, 1024, 2048])
+@pytest.mark.parametrize("axis", ["x", "y"])
+@pytest.mark.parametrize("bc_t", "PND")
+def test_every_fft_length(n, axis, bc_t):
+    """Each supported transform length on each axis, each transform type, ragged tiles."""
+    other = 4 if n >= 512 else 8
+    nx, ny = (n, other) if axis == "x" else (other, n)
+    nz = 3
+    combo = (bc_t + "N" + "D") if axis == "x" else ("D" + bc_t + "N")
+    shape = (nz, ny, nx)
+    h = (1.0 / nx, 1.0 / ny, 0.5)
+    f = wl.random_uniform(shape, n + (0 if axis == "x" else 1))
+    check(wl.Workload(f"len{n}{axis}{bc_t}", shape, h, wl.parse_bc(combo), f))
+
+
+def test_config1_both_variants():
+    for variant in ("mms", "uniform"):
+        w = wl.config1(variant)
+        u, ref = check(w)
+        if variant == "mms":       # eigenfunction: second-order accurate against the analytic solution
+            assert np.max(np.abs(u - w.u_exact)) < 5e-3
+
+
+@pytest.mark.parametrize("combo", wl.CONFIG2_COMBOS)
+@pytest.mark.parametrize("variant", ["mms", "normal"])
+def test_config2_128cubed(combo, variant):
+    check(wl.config2(combo, variant))
+
+
+@pytest.mark.parametrize("combo", ["PPN", "NNP", "DPD", "PDP", "NPN"])
+def test_tile_boundaries_and_long_z(combo):
+    """Several x tiles, several y tiles, nz spanning several checkpoint blocks with a ragged tail."""
+    shape = (67, 64, 128)
+    h = (1.0 / 128, 1.0 / 64, 1.0 / 67)
+    bc = wl.parse_bc(combo)
+    f = wl.random_normal(shape, 31, zero_mean=all(b in (0, 1) for b in bc))
+    check(wl.Workload(f"tiles-{combo}", shape, h, bc, f))
+
+
+def test_nz_extremes():
+    for nz in (2, 3, 16, 17, 1025):
+        for combo in ("PPN", "NDD", "DNP"):
+            shape = (nz, 8, 16)
+            f = wl.random_uniform(shape, nz)
+            check(wl.Workload(f"nz{nz}-{combo}", shape, (0.1, 0.1, 0.1), wl.parse_bc(combo), f))
+
+
+def test_config3_scaled_siblings():
+    for scale in (8, 4, 2):
+        check(wl.config3(scale))
+
+
+def test_config4_and_5_scaled():
+    check(wl.config4(64))
+    check(wl.config4(128, twin=True))
+    check(wl.config5(scale=8))
+
+
+@pytest.mark.parametrize("combo", ALL27)
+def test_second_order_convergence_on_gpu(combo):
+    """MMS error ratio 4 +- 0.3 on grid halving for every BC combination (north_star)."""
+    bc = wl.parse_bc(combo)
+    errs = []
+    for n in (16, 32, 64):
+        shape, h = (n, n, n), (1.0 / n,) * 3
+        f, u, _ = wl.mms(shape, h, bc)
+        uh = gpu_solve(f, h, bc)
+        if all(b in (0, 1) for b in bc):
+            u = u - u.mean()
+        errs.append(float(np.sqrt(np.mean((uh - u) ** 2))))
+    for coarse, fine in zip(errs[:-1], errs[1:]):
+        assert abs(coarse / fine - 4.0) <= 0.3, errs
