@@ -1,0 +1,342 @@
+#!/usr/bin/env python
+"""Benchmark of the direct Poisson solve (BASELINE.json metric: Gpoints/s per fp64 Poisson solve and
+% of HBM roofline at 512x512x256).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg3|cfg4|cfg5|cfg2]
+
+A "step" is one pp_solve: the whole hot path (x-fwd, y-fwd, z-solve, y-inv, x-inv) over one synthetic
+grid.  N > 1 runs N independent replicas (one process per GPU, no data-path collective -- DESIGN.md
+"replicas only"); value = points solved by all ranks / max-over-ranks device time.
+
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for the definition of every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Gpoints/s per fp64 Poisson solve"
+UNIT = "Gpoints/s"
+BYTES_PER_POINT_SOLVE = 80.0     # 5 passes x (8 B read + 8 B write)
+BYTES_PER_POINT_KERNEL = 16.0    # one pass
+FALLBACK_HBM_GBS = 6650.0        # /opt/skills/guides/B200_PROFILING.md
+
+
+def workload_by_name(name):
+    from paper_1909_05423_b200 import workloads as wl
+    if name == "cfg3":
+        return wl.config3()
+    if name == "cfg4":
+        return wl.config4()
+    if name == "cfg5":
+        return wl.config5()
+    if name == "cfg2":
+        return wl.config2("PPN", "normal")
+    if name == "cfg1":
+        return wl.config1("uniform")
+    raise SystemExit(f"unknown workload {name}")
+
+
+def describe(w):
+    nz, ny, nx = w.shape
+    bc = "".join("PND"[b] for b in w.bc)
+    return f"{nx}x{ny}x{nz} fp64, bc(x,y,z)={bc}, {w.name}"
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def committed_traffic(kernel):
+    """dram bytes per launch of `kernel` from the committed ncu --set full summary, or None."""
+    path = os.path.join(ROOT, "profiles", "r01_dram_traffic.csv")
+    try:
+        with open(path) as fh:
+            for line in fh:
+                t = [s.strip() for s in line.split(",")]
+                if len(t) >= 2 and t[0] == kernel:
+                    return float(t[1])
+    except Exception:
+        pass
+    return None
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown",
+               0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting"}
+
+    def __init__(self, index, period=0.01):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.stop_flag = threading.Event()
+        self.mhz, self.reasons, self.max_mhz, self.ok = [], set(), None, False
+
+    def run(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+            while not self.stop_flag.is_set():
+                self.mhz.append(int(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)))
+                try:
+                    mask = int(pynvml.nvmlDeviceGetCurrentClocksEventReasons(h))
+                except Exception:
+                    mask = int(pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(h))
+                for bit, name in self.REASONS.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+                time.sleep(self.period)
+        except Exception as exc:  # pragma: no cover
+            self.error = repr(exc)
+
+    def result(self):
+        if not self.ok or not self.mhz:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"], "samples": 0}
+        s = sorted(self.mhz)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+def physical_gpu_index(local_rank):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+# ------------------------------------------------------------------------------------------
+# the oracle arm (cpu_baseline and --impl reference)
+# ------------------------------------------------------------------------------------------
+def oracle_sample(w, step_seconds=18.0):
+    """Times the oracle, as it stands, on a bounded sample of workload `w`: the full x-y extent and
+    all boundary conditions, with as many z planes as fit the budget (per-point cost of the oracle is
+    flat in nz: the transforms are per plane, Thomas is O(nz) per mode)."""
+    import numpy as np
+    from oracle import poisson_oracle as po
+    nz, ny, nx = w.shape
+    def probe(n):
+        f = np.ascontiguousarray(w.f[:n])
+        t0 = time.perf_counter()
+        po.solve(f, w.h, w.bc)
+        return time.perf_counter() - t0
+
+    n1, n2 = min(nz, 2), min(nz, 10)
+    probe(n1)                                     # first call pays the BLAS start-up
+    t1, t2 = probe(n1), probe(n2)
+    per_plane = max((t2 - t1) / max(n2 - n1, 1), 1e-6)
+    fixed = max(t1 - per_plane * n1, 0.0)
+    target_nz = int(max(2, min(nz, (step_seconds - fixed) / per_plane)))
+    sample = {"nz": target_nz, "ny": ny, "nx": nx,
+              "text": (f"oracle.poisson_oracle.solve on the first {target_nz} of {nz} z-planes of the workload "
+                       f"({nx}x{ny}x{target_nz}, same spacings and BCs), one solve")}
+    return sample
+
+
+def time_oracle(w, sample):
+    import numpy as np
+    from oracle import poisson_oracle as po
+    f = np.ascontiguousarray(w.f[: sample["nz"]])
+    t0 = time.perf_counter()
+    po.solve(f, w.h, w.bc)
+    dt = time.perf_counter() - t0
+    return f.size / dt / 1e9, dt
+
+
+def blas_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [int(i.get("num_threads", 1)) for i in threadpool_info() if i.get("user_api") == "blas"]
+        if n:
+            return max(n)
+    except Exception:
+        pass
+    return len(os.sched_getaffinity(0))
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    w = workload_by_name(args.workload)
+    sample = oracle_sample(w, step_seconds=150.0 / max(1, args.steps + args.warmup))
+    for _ in range(args.warmup):
+        time_oracle(w, sample)
+    vals, secs = [], []
+    for _ in range(args.steps):
+        v, dt = time_oracle(w, sample)
+        vals.append(v)
+        secs.append(dt)
+    total_pts = sample["nz"] * sample["ny"] * sample["nx"] * args.steps
+    value = total_pts / sum(secs) / 1e9
+    cores = blas_threads()
+    out = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(secs) / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": describe(w), "sample": sample["text"]},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample["text"]},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------
+# the CUDA arm
+# ------------------------------------------------------------------------------------------
+def run_cuda(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import paper_1909_05423_b200 as pp
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local_rank)
+    distributed = world > 1
+    if distributed:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if distributed:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = workload_by_name(args.workload)
+    nz, ny, nx = w.shape
+    npts = w.n_points
+    plan = pp.Plan(nx, ny, nz, *w.h, w.bc)
+    f = torch.from_numpy(w.f).cuda()
+    u = torch.empty_like(f)
+    stream = torch.cuda.current_stream()
+
+    for _ in range(max(args.warmup, 3)):
+        plan.solve(f, u)
+    barrier()
+
+    # ---- timed region: K solves, inputs resident in HBM (f, u: 2 x N x 8 B, far larger than L2)
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    sampler.start()
+    time.sleep(0.05)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        plan.solve(f, u)
+    e1.record(stream)
+    barrier()
+    sampler.stop_flag.set()
+    sampler.join()
+    ms_total = e0.elapsed_time(e1)
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if distributed:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * npts / (ms_step * 1e-3) / 1e9
+
+    # ---- per-kernel durations over the same number of steps (CUDA events on the launching stream)
+    plan.set_profiling(True)
+    sums = dict.fromkeys(pp.KERNEL_NAMES, 0.0)
+    barrier()
+    for _ in range(args.steps):
+        plan.solve(f, u)
+        for k, v in plan.last_kernel_ms().items():
+            sums[k] += v
+    plan.set_profiling(False)
+    kernel_ms = {k: v / args.steps for k, v in sums.items()}
+
+    # ---- end to end through the host-buffer entry point (pinned host memory, H2D + solve + D2H)
+    e2e_steps = max(3, min(args.steps, 10))
+    fh = torch.from_numpy(w.f).pin_memory()
+    uh = torch.empty_like(fh).pin_memory()
+    plan.solve_host(fh, uh)
+    barrier()
+    e0.record(stream)
+    for _ in range(e2e_steps):
+        plan.solve_host(fh, uh)
+    e1.record(stream)
+    barrier()
+    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+    if distributed:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_ms = float(t.item()) / e2e_steps
+    e2e_value = world * npts / (e2e_ms * 1e-3) / 1e9
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        dom = max(kernel_ms, key=kernel_ms.get)
+        achieved = BYTES_PER_POINT_KERNEL * npts / (kernel_ms[dom] * 1e-3) / 1e9
+        solve_gbs = BYTES_PER_POINT_SOLVE * npts / (ms_step * 1e-3) / 1e9
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": describe(w), "parallelism": f"replicas x{world} (no collective)",
+                       "l2_policy": "inputs larger than L2 (f and u are %d MiB each)" % (npts * 8 >> 20),
+                       "in_place": False},
+            "clocks": sampler.result(),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": npts * 8, "d2h_bytes_per_step": npts * 8,
+                    "ms_per_step": e2e_ms, "steps": e2e_steps, "api": "pp_solve_host (pinned host buffers)"},
+            "gpu_launches": 5 * args.steps,
+            "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "traffic": committed_traffic(dom), "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": BYTES_PER_POINT_KERNEL * npts},
+            "roofline_solve": {"bound": "hbm", "achieved": solve_gbs, "peak": peak, "unit": "GB/s",
+                               "frac": solve_gbs / peak, "bytes_per_point": BYTES_PER_POINT_SOLVE,
+                               "frac_of_nominal_8TBs": solve_gbs / 8000.0},
+            "kernel_ms": kernel_ms,
+            "kernel_gbs": {k: BYTES_PER_POINT_KERNEL * npts / (v * 1e-3) / 1e9 for k, v in kernel_ms.items()},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            sample = oracle_sample(w, step_seconds=18.0)
+            v, dt = time_oracle(w, sample)
+            out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
+                                   "sample": sample["text"], "seconds": dt}
+        print(json.dumps(out))
+    plan.destroy()
+    if distributed:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="cfg3", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
