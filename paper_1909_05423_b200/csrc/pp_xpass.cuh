@@ -42,6 +42,10 @@ struct GroupSync {
 
 __device__ __forceinline__ double sgn_of(int i) { return (i & 1) ? -1.0 : 1.0; }
 
+#ifndef PP_X_MINB
+#define PP_X_MINB 4
+#endif
+
 template <int N>
 struct XCfg {
     static constexpr int P = FftCfg<N>::P;
@@ -54,7 +58,7 @@ struct XCfg {
 // forward: real rows -> spectral rows
 // ------------------------------------------------------------------------------------------
 template <int N>
-__global__ void __launch_bounds__(XCfg<N>::THREADS)
+__global__ void __launch_bounds__(XCfg<N>::THREADS, PP_X_MINB)
 xpass_fwd_kernel(const double *in, double *out, long long npairs, int bc,
                  const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
     using C = FftCfg<N>;
@@ -143,7 +147,7 @@ xpass_fwd_kernel(const double *in, double *out, long long npairs, int bc,
 // inverse: spectral rows -> real rows
 // ------------------------------------------------------------------------------------------
 template <int N>
-__global__ void __launch_bounds__(XCfg<N>::THREADS)
+__global__ void __launch_bounds__(XCfg<N>::THREADS, PP_X_MINB)
 xpass_inv_kernel(const double *in, double *out, long long npairs, int bc,
                  const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
     using C = FftCfg<N>;

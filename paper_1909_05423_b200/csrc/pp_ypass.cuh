@@ -34,18 +34,26 @@ struct SyncCta {
     __device__ __forceinline__ void operator()() const { __syncthreads(); }
 };
 
+#ifndef PP_Y_T
+#define PP_Y_T 8          // double2 columns per CTA for N <= 512 (128-byte row segments)
+#endif
+#ifndef PP_Y_MINB
+#define PP_Y_MINB 2       // __launch_bounds__ min CTAs per SM (caps registers) for CTAs of <= 512 threads
+#endif
+
 template <int N>
 struct YCfg {
     static constexpr int P = FftCfg<N>::P;
-    static constexpr int T = (N <= 512) ? 8 : 4;        // double2 columns per CTA (128 / 64 B row segments)
+    static constexpr int T = (N <= 512) ? PP_Y_T : 4;   // double2 columns per CTA
     static constexpr int THREADS = T * P;
+    static constexpr int MINB = (THREADS <= 512) ? PP_Y_MINB : 1;
     static constexpr size_t SMEM = size_t(T) * FftCfg<N>::SMEM_ELEMS * sizeof(double2);
 };
 
 __device__ __forceinline__ double2 dscale(double a, double2 v) { return make_double2(a * v.x, a * v.y); }
 
 template <int N>
-__global__ void __launch_bounds__(YCfg<N>::THREADS)
+__global__ void __launch_bounds__(YCfg<N>::THREADS, YCfg<N>::MINB)
 ypass_fwd_kernel(double2 *w, int nxh, int bc, int complex_cols,
                  const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
     using C = FftCfg<N>;
@@ -135,7 +143,7 @@ ypass_fwd_kernel(double2 *w, int nxh, int bc, int complex_cols,
 }
 
 template <int N>
-__global__ void __launch_bounds__(YCfg<N>::THREADS)
+__global__ void __launch_bounds__(YCfg<N>::THREADS, YCfg<N>::MINB)
 ypass_inv_kernel(double2 *w, int nxh, int bc, int complex_cols,
                  const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
     using C = FftCfg<N>;

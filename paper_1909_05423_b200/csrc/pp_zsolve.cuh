@@ -33,39 +33,73 @@ struct ZParams {
     double scale;            // dz^2 / (nx ny): rhs scaling incl. the inverse-transform normalisation
     const double *sx;        // [nx]  dz^2 lam_x(kx(ix)) / dx^2
     const double *sy;        // [ny]  dz^2 lam_y(ky(j))  / dy^2
-    double *zero_scratch;    // [nz]  pivots of the zero-mode line
+    double *zero_scratch;    // [nz]  scratch line for the zero-mode solve
 };
 
 constexpr int Z_MAX_CK = 64;   // checkpoints per line
 
-// Serial solve of the singular (0,0) line by one thread (R11):
-// r <- (r - mean r) * scale; x_0 = 0; Thomas on rows 1..nz-1 of L_z; x <- x - mean x.
-__device__ __noinline__ void zero_mode_line(double *col, size_t plane, int nz, int bcz, double scale, double *gam) {
-    double sum = 0.0;
-    for (int k = 0; k < nz; ++k) sum += col[k * plane];
-    const double mean = sum / nz;
-    const double blast = (bcz == 1) ? -1.0 : -2.0;     // Neumann: -1; periodic: corners dropped with row 0
-    if (nz >= 2) {
-        double beta = (nz == 2) ? blast : -2.0;
-        double x = ((col[plane] - mean) * scale) / beta;
-        col[plane] = x;
-        for (int k = 2; k < nz; ++k) {
-            const double g = 1.0 / beta;
-            gam[k] = g;
-            beta = ((k == nz - 1) ? blast : -2.0) - g;
-            x = ((col[k * plane] - mean) * scale - x) / beta;
-            col[k * plane] = x;
-        }
-        for (int k = nz - 2; k >= 1; --k) {
-            x = col[k * plane] - gam[k + 1] * x;
-            col[k * plane] = x;
-        }
+// The singular (0,0) line, solved cooperatively by one full warp (R11):
+//   r <- (r - mean r) * scale;  pin x_0 = 0 and drop row 0;  solve rows 1..nz-1 of L_z;  x <- x - mean x.
+// With s = 0 the rows are pure second differences, so the pinned system is solved by two running
+// sums instead of a serial elimination (d_k = x_k - x_{k-1}):
+//   Neumann :  d_k = -sum_{m >= k} r_m                      (last row: x_{n-2} - x_{n-1} = r_{n-1})
+//   periodic:  d_k = d_1 + sum_{1 <= m < k} r_m,  d_1 fixed by x_n = x_0 = 0
+//   x_k = sum_{1 <= m <= k} d_m.
+// Each lane scans a contiguous chunk; chunk totals are combined with warp shuffles.  `tmp` is a
+// plan-owned scratch line of nz doubles.  All 32 lanes must call this.
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+// exclusive prefix of per-lane totals (lane order ascending)
+__device__ __forceinline__ double warp_excl_scan(double v, int lane) {
+    double inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const double t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
     }
-    col[0] = 0.0;
-    double s2 = 0.0;
-    for (int k = 1; k < nz; ++k) s2 += col[k * plane];
-    const double m2 = s2 / nz;
-    for (int k = 0; k < nz; ++k) col[k * plane] -= m2;
+    return inc - v;
+}
+
+__device__ __noinline__ void zero_mode_line(double *col, size_t plane, int nz, int bcz, double scale, double *tmp) {
+    const int lane = threadIdx.x & 31;
+    const int c = (nz + 31) / 32;
+    const int k0 = min(lane * c, nz), k1 = min(k0 + c, nz);
+    // mean of r
+    double acc = 0.0;
+    for (int k = k0; k < k1; ++k) { const double r = col[(size_t)k * plane] * scale; tmp[k] = r; acc += r; }
+    const double mean = warp_sum(acc) / nz;
+    // running sums of (r - mean) over rows 1..nz-1  ->  d_k in tmp[k]
+    double tot = 0.0;
+    for (int k = max(k0, 1); k < k1; ++k) tot += tmp[k] - mean;
+    const double before = warp_excl_scan(tot, lane);          // sum over lanes below
+    const double all = __shfl_sync(0xffffffffu, before + tot, 31);
+    __syncwarp();
+    if (bcz == 1) {
+        // Neumann: d_k = -(sum_{m >= k} r_m) = -(all - sum_{m < k} r_m)
+        double run = before;
+        for (int k = max(k0, 1); k < k1; ++k) { const double r = tmp[k] - mean; tmp[k] = -(all - run); run += r; }
+    } else {
+        // periodic: d_k = d_1 + S_{k-1}, S_j = sum_{1 <= m <= j} r_m; first store S_{k-1}, then add d_1
+        double run = before;
+        for (int k = max(k0, 1); k < k1; ++k) { const double r = tmp[k] - mean; tmp[k] = run; run += r; }
+        // x_n = 0:  n d_1 + sum_{k=1..n} S_{k-1} = 0, S_{n-1} = all
+        double ssum = 0.0;
+        for (int k = max(k0, 1); k < k1; ++k) ssum += tmp[k];
+        const double d1 = -(warp_sum(ssum) + all) / nz;
+        for (int k = max(k0, 1); k < k1; ++k) tmp[k] += d1;
+    }
+    __syncwarp();
+    // x_k = sum_{1 <= m <= k} d_m
+    double dt = 0.0;
+    for (int k = max(k0, 1); k < k1; ++k) dt += tmp[k];
+    double run = warp_excl_scan(dt, lane);
+    double xs = 0.0;
+    for (int k = max(k0, 1); k < k1; ++k) { run += tmp[k]; tmp[k] = run; xs += run; }
+    const double xmean = warp_sum(xs) / nz;                   // x_0 = 0 contributes nothing
+    for (int k = k0; k < k1; ++k) col[(size_t)k * plane] = ((k == 0) ? 0.0 : tmp[k]) - xmean;
 }
 
 // Neumann / Dirichlet in z.  One thread per real element of a plane.
@@ -74,15 +108,15 @@ __global__ void __launch_bounds__(256)
 zsolve_thomas_kernel(double *w, ZParams p) {
     const size_t plane = (size_t)p.nx * p.ny;
     const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= plane) return;
-    const int ix = (int)(e % p.nx), j = (int)(e / p.nx);
-    const bool pin = p.singular && e == 0;
+    const bool live = e < plane;                              // dead threads run along (warp-wide zero-mode solve) but never store
+    const int ix = live ? (int)(e % p.nx) : 0, j = live ? (int)(e / p.nx) : 0;
+    const bool pin = !live || (p.singular && e == 0);
     const double s = pin ? -1.0 : (p.sx[ix] + p.sy[j]);      // pinned line: placeholder, results discarded
     const double bint = -2.0 + s;
     const double bend = ((p.bcz == 1) ? -1.0 : -3.0) + s;
     const int nz = p.nz;
     const double scale = p.scale;
-    double *col = w + e;
+    double *col = w + (live ? e : 0);
     double ck[Z_MAX_CK];
 
     // forward sweep, in blocks of CB rows: batch the loads, then run the chain
@@ -126,7 +160,8 @@ zsolve_thomas_kernel(double *w, ZParams p) {
             }
         }
     }
-    if (pin) zero_mode_line(col, plane, nz, p.bcz, scale, p.zero_scratch);
+    // the warp that owns element 0 solves the singular line together (block 0, warp 0: all lanes alive)
+    if (p.singular && e < 32) zero_mode_line(w, plane, nz, p.bcz, scale, p.zero_scratch);
 }
 
 // Periodic in z: Sherman-Morrison, "two solves".  With gamma = -b:
@@ -139,9 +174,9 @@ __global__ void __launch_bounds__(256)
 zsolve_cyclic_kernel(double *w, ZParams p) {
     const size_t plane = (size_t)p.nx * p.ny;
     const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= plane) return;
-    const int ix = (int)(e % p.nx), j = (int)(e / p.nx);
-    const bool pin = p.singular && e == 0;
+    const bool live = e < plane;
+    const int ix = live ? (int)(e % p.nx) : 0, j = live ? (int)(e / p.nx) : 0;
+    const bool pin = !live || (p.singular && e == 0);
     const double s = pin ? -1.0 : (p.sx[ix] + p.sy[j]);
     const double b = -2.0 + s;
     const double gamma = -b;
@@ -149,7 +184,7 @@ zsolve_cyclic_kernel(double *w, ZParams p) {
     const double blast = b - 1.0 / gamma;         // b + 1/b
     const int nz = p.nz;
     const double scale = p.scale;
-    double *col = w + e;
+    double *col = w + (live ? e : 0);
     double ckg[Z_MAX_CK], ckq[Z_MAX_CK];
 
     double g = 0.0, xp = 0.0, qp = 0.0;
@@ -208,7 +243,8 @@ zsolve_cyclic_kernel(double *w, ZParams p) {
         }
         if (sweep == 0) fac = (x + xlast / gamma) / (1.0 + q + qlast / gamma);
     }
-    if (pin) zero_mode_line(col, plane, nz, p.bcz, scale, p.zero_scratch);
+    // the warp that owns element 0 solves the singular line together (block 0, warp 0: all lanes alive)
+    if (p.singular && e < 32) zero_mode_line(w, plane, nz, p.bcz, scale, p.zero_scratch);
 }
 
 }  // namespace pp
