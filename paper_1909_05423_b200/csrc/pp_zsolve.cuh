@@ -38,6 +38,46 @@ struct ZParams {
 
 constexpr int Z_MAX_CK = 64;   // checkpoints per line
 
+// L2 eviction-priority hints (createpolicy + .L2::cache_hint).  The forward sweep's x' values are
+// re-read by the backward sweep: they are stored "evict_last" so they survive in the 126 MB L2,
+// while the streams that are touched once (right-hand side in, solution out) are "evict_first".
+#ifndef PP_Z_HINTS
+#define PP_Z_HINTS 1
+#endif
+#ifndef PP_Z_THREADS
+#define PP_Z_THREADS 256
+#endif
+#ifndef PP_Z_MINB
+#define PP_Z_MINB 2
+#endif
+struct ZPolicy {
+    unsigned long long first, last;
+    __device__ __forceinline__ ZPolicy() {
+#if PP_Z_HINTS
+        asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(first));
+        asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(last));
+#else
+        first = last = 0;
+#endif
+    }
+};
+__device__ __forceinline__ double ld_hint(const double *p, unsigned long long pol) {
+#if PP_Z_HINTS
+    double v;
+    asm volatile("ld.global.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol));
+    return v;
+#else
+    return *p;
+#endif
+}
+__device__ __forceinline__ void st_hint(double *p, double v, unsigned long long pol) {
+#if PP_Z_HINTS
+    asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(p), "d"(v), "l"(pol) : "memory");
+#else
+    *p = v;
+#endif
+}
+
 // The singular (0,0) line, solved cooperatively by one full warp (R11):
 //   r <- (r - mean r) * scale;  pin x_0 = 0 and drop row 0;  solve rows 1..nz-1 of L_z;  x <- x - mean x.
 // With s = 0 the rows are pure second differences, so the pinned system is solved by two running
@@ -104,7 +144,7 @@ __device__ __noinline__ void zero_mode_line(double *col, size_t plane, int nz, i
 
 // Neumann / Dirichlet in z.  One thread per real element of a plane.
 template <int CB>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(PP_Z_THREADS, PP_Z_MINB)
 zsolve_thomas_kernel(double *w, ZParams p) {
     const size_t plane = (size_t)p.nx * p.ny;
     const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -117,6 +157,7 @@ zsolve_thomas_kernel(double *w, ZParams p) {
     const int nz = p.nz;
     const double scale = p.scale;
     double *col = w + (live ? e : 0);
+    const ZPolicy pol;
     double ck[Z_MAX_CK];
 
     // forward sweep, in blocks of CB rows: batch the loads, then run the chain
@@ -125,7 +166,7 @@ zsolve_thomas_kernel(double *w, ZParams p) {
         ck[k0 / CB] = g;
         double r[CB];
 #pragma unroll
-        for (int i = 0; i < CB; ++i) r[i] = (k0 + i < nz) ? col[(size_t)(k0 + i) * plane] : 0.0;
+        for (int i = 0; i < CB; ++i) r[i] = (k0 + i < nz) ? ld_hint(col + (size_t)(k0 + i) * plane, pol.first) : 0.0;
 #pragma unroll
         for (int i = 0; i < CB; ++i) {
             const int k = k0 + i;
@@ -133,7 +174,7 @@ zsolve_thomas_kernel(double *w, ZParams p) {
                 const double bk = (k == 0 || k == nz - 1) ? bend : bint;
                 g = 1.0 / (bk - g);
                 xp = (r[i] * scale - xp) * g;
-                if (!pin) col[(size_t)k * plane] = xp;
+                if (!pin) st_hint(col + (size_t)k * plane, xp, pol.last);
             }
         }
     }
@@ -143,7 +184,7 @@ zsolve_thomas_kernel(double *w, ZParams p) {
         double gl[CB], r[CB];
         double gg = ck[k0 / CB];
 #pragma unroll
-        for (int i = 0; i < CB; ++i) r[i] = (k0 + i < nz - 1) ? col[(size_t)(k0 + i) * plane] : 0.0;
+        for (int i = 0; i < CB; ++i) r[i] = (k0 + i < nz - 1) ? ld_hint(col + (size_t)(k0 + i) * plane, pol.first) : 0.0;
 #pragma unroll
         for (int i = 0; i < CB; ++i) {
             const int k = k0 + i;
@@ -156,7 +197,7 @@ zsolve_thomas_kernel(double *w, ZParams p) {
             const int k = k0 + i;
             if (k < nz - 1) {
                 x = r[i] - gl[i] * x;
-                if (!pin) col[(size_t)k * plane] = x;
+                if (!pin) st_hint(col + (size_t)k * plane, x, pol.first);
             }
         }
     }
@@ -170,7 +211,7 @@ zsolve_thomas_kernel(double *w, ZParams p) {
 // q depends only on the mode, so it is never stored: it is recomputed next to the pivots.
 // Sweep 1 forward (x'), sweep 2 backward (x, and q to get the scalar), sweep 3 backward (u).
 template <int CB>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(PP_Z_THREADS, PP_Z_MINB)
 zsolve_cyclic_kernel(double *w, ZParams p) {
     const size_t plane = (size_t)p.nx * p.ny;
     const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -185,6 +226,7 @@ zsolve_cyclic_kernel(double *w, ZParams p) {
     const int nz = p.nz;
     const double scale = p.scale;
     double *col = w + (live ? e : 0);
+    const ZPolicy pol;
     double ckg[Z_MAX_CK], ckq[Z_MAX_CK];
 
     double g = 0.0, xp = 0.0, qp = 0.0;
@@ -193,7 +235,7 @@ zsolve_cyclic_kernel(double *w, ZParams p) {
         ckq[k0 / CB] = qp;
         double r[CB];
 #pragma unroll
-        for (int i = 0; i < CB; ++i) r[i] = (k0 + i < nz) ? col[(size_t)(k0 + i) * plane] : 0.0;
+        for (int i = 0; i < CB; ++i) r[i] = (k0 + i < nz) ? ld_hint(col + (size_t)(k0 + i) * plane, pol.first) : 0.0;
 #pragma unroll
         for (int i = 0; i < CB; ++i) {
             const int k = k0 + i;
@@ -203,7 +245,7 @@ zsolve_cyclic_kernel(double *w, ZParams p) {
                 g = 1.0 / (bk - g);
                 xp = (r[i] * scale - xp) * g;
                 qp = (wk - qp) * g;
-                if (!pin) col[(size_t)k * plane] = xp;
+                if (!pin) st_hint(col + (size_t)k * plane, xp, pol.last);
             }
         }
     }
@@ -216,7 +258,7 @@ zsolve_cyclic_kernel(double *w, ZParams p) {
             double gl[CB], ql[CB], r[CB];
             double gg = ckg[k0 / CB], qq = ckq[k0 / CB];
 #pragma unroll
-            for (int i = 0; i < CB; ++i) r[i] = (k0 + i < nz - 1) ? col[(size_t)(k0 + i) * plane] : 0.0;
+            for (int i = 0; i < CB; ++i) r[i] = (k0 + i < nz - 1) ? ld_hint(col + (size_t)(k0 + i) * plane, sweep == 0 ? pol.last : pol.first) : 0.0;
 #pragma unroll
             for (int i = 0; i < CB; ++i) {
                 const int k = k0 + i;
@@ -234,9 +276,9 @@ zsolve_cyclic_kernel(double *w, ZParams p) {
                     q = ql[i] - gl[i] * q;
                     if (sweep == 0) {
                         x = r[i] - gl[i] * x;                  // r holds x'_k
-                        if (!pin) col[(size_t)k * plane] = x;
+                        if (!pin) st_hint(col + (size_t)k * plane, x, pol.last);
                     } else {
-                        if (!pin) col[(size_t)k * plane] = r[i] - fac * q;   // r holds x_k
+                        if (!pin) st_hint(col + (size_t)k * plane, r[i] - fac * q, pol.first);   // r holds x_k
                     }
                 }
             }
