@@ -62,7 +62,7 @@ def measured_peak():
 
 def committed_traffic(kernel):
     """dram bytes per launch of `kernel` from the committed ncu --set full summary, or None."""
-    path = os.path.join(ROOT, "profiles", "r01_dram_traffic.csv")
+    path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
     try:
         with open(path) as fh:
             for line in fh:
