@@ -202,6 +202,26 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------
+# N > 1: replicas only -- the only cross-rank step is the timing reduction
+# ------------------------------------------------------------------------------------------
+def max_over_ranks(ms: float, device="cpu") -> float:
+    """Slowest rank's device time.  Uses the default process group if one is initialised (NCCL on
+    the GPU box, gloo in the CPU tests); a single process returns its own time."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms)
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_gpoints(world: int, npts_per_rank: int, ms_step: float) -> float:
+    """Every rank solves its own grid (weak scaling): points solved by all ranks / slowest rank's time."""
+    return world * npts_per_rank / (ms_step * 1e-3) / 1e9
+
+
+# ------------------------------------------------------------------------------------------
 # the CUDA arm
 # ------------------------------------------------------------------------------------------
 def run_cuda(args):
@@ -250,13 +270,9 @@ def run_cuda(args):
     barrier()
     sampler.stop_flag.set()
     sampler.join()
-    ms_total = e0.elapsed_time(e1)
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if distributed:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total = float(t.item())
+    ms_total = max_over_ranks(e0.elapsed_time(e1), "cuda")
     ms_step = ms_total / args.steps
-    value = world * npts / (ms_step * 1e-3) / 1e9
+    value = whole_job_gpoints(world, npts, ms_step)
 
     # ---- per-kernel durations over the same number of steps (CUDA events on the launching stream)
     plan.set_profiling(True)
@@ -280,11 +296,8 @@ def run_cuda(args):
         plan.solve_host(fh, uh)
     e1.record(stream)
     barrier()
-    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-    if distributed:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_ms = float(t.item()) / e2e_steps
-    e2e_value = world * npts / (e2e_ms * 1e-3) / 1e9
+    e2e_ms = max_over_ranks(e0.elapsed_time(e1), "cuda") / e2e_steps
+    e2e_value = whole_job_gpoints(world, npts, e2e_ms)
 
     if rank == 0:
         peak, peak_src = measured_peak()
