@@ -24,7 +24,7 @@ struct pp_plan {
     int device;
     int singular;
     double scale;
-    double2 *tw_x, *tw_y;      // exp(-2 pi i m / n), m in [0, n)
+    double2 *tw_x, *tw_y;      // per-stage FFT twiddle tables (pp_fft.cuh, tw_stage_offset)
     double2 *ptw_x, *ptw_y;    // exp(-i pi m / (2n)), m in [0, n]
     double *sx, *sy;           // dz^2 lam / h^2 per packed position
     double *zero_scratch;      // [nz]
@@ -45,11 +45,17 @@ const long double PI_L = 3.14159265358979323846264338327950288L;
 bool pow2_in_range(int n) { return n >= 4 && n <= 2048 && (n & (n - 1)) == 0; }
 
 void make_twiddles(int n, std::vector<double2> &tw, std::vector<double2> &ptw) {
-    tw.resize(n);
+    tw.assign(tw_table_elems(n), make_double2(1.0, 0.0));
     ptw.resize(n + 1);
-    for (int m = 0; m < n; ++m) {
-        const long double a = 2.0L * PI_L * (long double)m / (long double)n;
-        tw[m] = make_double2((double)cosl(a), (double)(-sinl(a)));
+    // stage with NS (radix 8): rows r = 1, 2, 4 of W_n^(k r stride), stride = n / (8 NS), k in [0, NS)
+    for (int ns = first_radix(n); ns < n; ns *= 8) {
+        const int off = tw_stage_offset(n, ns), stride = n / (8 * ns);
+        for (int ri = 0; ri < 3; ++ri)
+            for (int k = 0; k < ns; ++k) {
+                const long long e = ((long long)k * (1 << ri) * stride) % n;
+                const long double a = 2.0L * PI_L * (long double)e / (long double)n;
+                tw[off + ri * ns + k] = make_double2((double)cosl(a), (double)(-sinl(a)));
+            }
     }
     for (int m = 0; m <= n; ++m) {
         const long double a = PI_L * (long double)m / (2.0L * (long double)n);

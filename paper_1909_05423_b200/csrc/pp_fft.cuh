@@ -32,6 +32,21 @@ struct FftCfg {
     static constexpr int SMEM_ELEMS = N + N / 8;   // double2 elements per transform incl. padding
 };
 
+// Stage twiddle tables.  Every stage after the first is radix 8 and multiplies input r of butterfly
+// j by W_N^(k r STRIDE), k = j mod NS, STRIDE = N / (8 NS).  The plan stores, per stage, the three
+// rows r = 1, 2, 4 as [r][k] -- contiguous in k, so a warp's 16-byte loads touch NS*16 contiguous
+// bytes (one L1 line for NS = 8, four for NS >= 32) instead of lines STRIDE*16 bytes apart; the other
+// powers are products.  Stage with NS starts at element 3 * (sum of the earlier stages' NS).
+__host__ __device__ constexpr int first_radix(int n) {
+    return (ilog2(n) % 3 == 0) ? 8 : ((ilog2(n) % 3 == 1) ? 2 : 4);
+}
+__host__ __device__ constexpr int tw_stage_offset(int n, int NS) {
+    int off = 0;
+    for (int ns = first_radix(n); ns < NS; ns *= 8) off += 3 * ns;
+    return off;
+}
+__host__ __device__ constexpr int tw_table_elems(int n) { return tw_stage_offset(n, n) > 0 ? tw_stage_offset(n, n) : 1; }
+
 __device__ __forceinline__ int pad8(int i) { return i + (i >> 3); }
 
 __device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
@@ -113,26 +128,21 @@ __device__ __forceinline__ void fft_stage(double2 (&v)[FftCfg<N>::E], int t, dou
         for (int r = 0; r < R; ++r) x[r] = v[b + B * r];
         const int k = j & (NS - 1);
         if constexpr (NS > 1) {
-            constexpr int STRIDE = N / (NS * R);
-            // W^(k r STRIDE): load the power-of-two multiples, build the rest with one product each
-            double2 w1 = __ldg(&tw[k * STRIDE]);
-            if (DIR == INV) w1 = cconj(w1);
+            static_assert(R == 8, "every stage after the first is radix 8");
+            // W^(k r STRIDE): load r = 1, 2, 4 from the stage table, build the rest with one product each
+            const double2 *ts = tw + tw_stage_offset(N, NS);
+            double2 w1 = __ldg(&ts[k]);
+            double2 w2 = __ldg(&ts[NS + k]);
+            double2 w4 = __ldg(&ts[2 * NS + k]);
+            if (DIR == INV) { w1 = cconj(w1); w2 = cconj(w2); w4 = cconj(w4); }
+            const double2 w3 = cmul(w1, w2);
             x[1] = cmul(x[1], w1);
-            if constexpr (R >= 4) {
-                double2 w2 = __ldg(&tw[2 * k * STRIDE]);
-                if (DIR == INV) w2 = cconj(w2);
-                double2 w3 = cmul(w1, w2);
-                x[2] = cmul(x[2], w2);
-                x[3] = cmul(x[3], w3);
-                if constexpr (R == 8) {
-                    double2 w4 = __ldg(&tw[4 * k * STRIDE]);
-                    if (DIR == INV) w4 = cconj(w4);
-                    x[4] = cmul(x[4], w4);
-                    x[5] = cmul(x[5], cmul(w1, w4));
-                    x[6] = cmul(x[6], cmul(w2, w4));
-                    x[7] = cmul(x[7], cmul(w3, w4));
-                }
-            }
+            x[2] = cmul(x[2], w2);
+            x[3] = cmul(x[3], w3);
+            x[4] = cmul(x[4], w4);
+            x[5] = cmul(x[5], cmul(w1, w4));
+            x[6] = cmul(x[6], cmul(w2, w4));
+            x[7] = cmul(x[7], cmul(w3, w4));
         }
         bfly<R, DIR>(x);
         if constexpr (LAST) {

@@ -93,9 +93,10 @@ xpass_fwd_kernel(const double *in, double *out, long long npairs, int bc,
 
     fft<N, FWD>(v, t, s, tw, lay, sync);
 
-    // ---- post-processing: Hermitian separation of the two rows, twiddle, store
+    // ---- post-processing: Hermitian separation of the two rows, twiddle, store.  The partner
+    // Z_{N-m} of m in (0, N/2) lives in the upper half, so only that half goes through shared memory.
 #pragma unroll
-    for (int q = 0; q < E; ++q) s[lay(t + q * P)] = v[q];
+    for (int q = E / 2; q < E; ++q) s[lay(t + q * P)] = v[q];
     sync();
     if (active) {
 #pragma unroll
@@ -164,18 +165,31 @@ xpass_inv_kernel(const double *in, double *out, long long npairs, int bc,
     const GroupSync<P, T> sync{f};
 
     double2 v[E];
+    if (bc == BC_P) {
+        // Every packed element (A_m, B_m), m in [0, N/2), is loaded once by the thread that owns Z_m;
+        // the mirrored Z_{N-m} = conj(A_m) + i conj(B_m) is handed to its owner through shared memory.
+#pragma unroll
+        for (int q = 0; q < E / 2; ++q) {
+            const int m = t + q * P;
+            const double2 A = *reinterpret_cast<const double2 *>(ra + 2 * m);
+            const double2 B = *reinterpret_cast<const double2 *>(rb + 2 * m);
+            if (m == 0) {                                              // (X_0, X_{N/2}) of both rows, all real
+                v[q] = make_double2(A.x, B.x);
+                s[lay(H)] = make_double2(A.y, B.y);
+            } else {
+                v[q] = make_double2(A.x - B.y, A.y + B.x);             // Z_m = A + i B
+                s[lay(N - m)] = make_double2(A.x + B.y, B.x - A.y);    // Z_{N-m}
+            }
+        }
+        sync();
+#pragma unroll
+        for (int q = E / 2; q < E; ++q) v[q] = s[lay(t + q * P)];
+        sync();
+    }
 #pragma unroll
     for (int q = 0; q < E; ++q) {
         const int m = t + q * P;
         if (bc == BC_P) {
-            double2 A, B;
-            if (m == 0)      { A = make_double2(ra[0], 0.0); B = make_double2(rb[0], 0.0); }
-            else if (m == H) { A = make_double2(ra[1], 0.0); B = make_double2(rb[1], 0.0); }
-            else if (m < H)  { A = *reinterpret_cast<const double2 *>(ra + 2 * m);
-                               B = *reinterpret_cast<const double2 *>(rb + 2 * m); }
-            else             { A = cconj(*reinterpret_cast<const double2 *>(ra + 2 * (N - m)));
-                               B = cconj(*reinterpret_cast<const double2 *>(rb + 2 * (N - m))); }
-            v[q] = make_double2(A.x - B.y, A.y + B.x);                 // Z = A + i B
         } else {
             double ya, yb, yap, ybp;
             if (bc == BC_N) {
@@ -194,7 +208,7 @@ xpass_inv_kernel(const double *in, double *out, long long npairs, int bc,
     }
     // all loads of this row pair are done before any thread of the group stores (in-place safe):
     // the FFT's exchanges synchronise the group; for single-stage transforms sync explicitly
-    if constexpr (C::R0 == N) sync();
+    if constexpr (C::R0 == N) { if (bc != BC_P) sync(); }
 
     fft<N, INV>(v, t, s, tw, lay, sync);
 

@@ -92,7 +92,7 @@ ypass_fwd_kernel(double2 *w, int nxh, int bc, int complex_cols,
         return;
     }
 #pragma unroll
-    for (int q = 0; q < E; ++q) smem[lay(t + q * P)] = v[q];
+    for (int q = E / 2; q < E; ++q) smem[lay(t + q * P)] = v[q];       // partners live in the upper half
     __syncthreads();
     if (!active) return;
     if (complex_cols && cp > 0) {
