@@ -171,33 +171,41 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
     zp.sx = p->sx; zp.sy = p->sy;
     zp.zero_scratch = p->zero_scratch;
     const size_t plane = (size_t)p->nx * p->ny;
-    constexpr int TH = PP_Z_THREADS;
-    const unsigned grid = (unsigned)((plane + TH - 1) / TH);
-#ifdef PP_Z_CB
-    const int cb = PP_Z_CB;
-#else
-    const int cb = (p->nz <= 16 * Z_MAX_CK) ? 16 : ((p->nz <= 32 * Z_MAX_CK) ? 32 : 64);
-#endif
 #ifndef PP_Z_DSMEM
 #define PP_Z_DSMEM 0
 #endif
-    const size_t ds = PP_Z_DSMEM;      // dummy dynamic shared memory: caps resident CTAs per SM
+#ifndef PP_Z_CB
+#define PP_Z_CB 16
+#endif
+    if (p->bcz != PP_BC_PERIODIC) {
+        // checkpoint table in shared memory: ceil(nz / CB) x TH doubles per CTA
+#define PP_ZT_LAUNCH(C, T)                                                                           \
+        do {                                                                                         \
+            const size_t ds = (size_t)(((p->nz + 1) / 2 + C - 1) / C) * T * sizeof(double) + PP_Z_DSMEM; \
+            if (int rc = set_smem(zsolve_thomas_kernel<C, T>, ds)) return rc;                        \
+            zsolve_thomas_kernel<C, T><<<(unsigned)((plane + T - 1) / T), T, ds, st>>>(w, zp);       \
+        } while (0)
+#ifdef PP_Z_TH
+        PP_ZT_LAUNCH(PP_Z_CB, PP_Z_TH);
+#else
+        PP_ZT_LAUNCH(PP_Z_CB, 128);
+#endif
+#undef PP_ZT_LAUNCH
+    } else {
+        constexpr int TH = PP_Z_THREADS;
+        const unsigned grid = (unsigned)((plane + TH - 1) / TH);
+        const int cb = (p->nz <= 16 * Z_MAX_CK) ? 16 : ((p->nz <= 32 * Z_MAX_CK) ? 32 : 64);
+        const size_t ds = PP_Z_DSMEM;      // dummy dynamic shared memory: caps resident CTAs per SM
 #define PP_Z_LAUNCH(K, C)                                                                        \
-    do {                                                                                         \
-        if (int rc = set_smem(K<C>, ds)) return rc;                                              \
-        K<C><<<grid, TH, ds, st>>>(w, zp);                                                       \
-    } while (0)
-    if (p->bcz == PP_BC_PERIODIC) {
+        do {                                                                                     \
+            if (int rc = set_smem(K<C>, ds)) return rc;                                          \
+            K<C><<<grid, TH, ds, st>>>(w, zp);                                                   \
+        } while (0)
         if (cb == 16)      PP_Z_LAUNCH(zsolve_cyclic_kernel, 16);
         else if (cb == 32) PP_Z_LAUNCH(zsolve_cyclic_kernel, 32);
         else               PP_Z_LAUNCH(zsolve_cyclic_kernel, 64);
-    } else {
-        if (cb == 8)       PP_Z_LAUNCH(zsolve_thomas_kernel, 8);
-        else if (cb == 16) PP_Z_LAUNCH(zsolve_thomas_kernel, 16);
-        else if (cb == 32) PP_Z_LAUNCH(zsolve_thomas_kernel, 32);
-        else               PP_Z_LAUNCH(zsolve_thomas_kernel, 64);
-    }
 #undef PP_Z_LAUNCH
+    }
     return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
 }
 

@@ -24,6 +24,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include "pp_async.cuh"
+
 namespace pp {
 
 struct ZParams {
@@ -142,12 +144,125 @@ __device__ __noinline__ void zero_mode_line(double *col, size_t plane, int nz, i
     for (int k = k0; k < k1; ++k) col[(size_t)k * plane] = ((k == 0) ? 0.0 : tmp[k]) - xmean;
 }
 
-// Neumann / Dirichlet in z.  One thread per real element of a plane.
-template <int CB>
-__global__ void __launch_bounds__(PP_Z_THREADS, PP_Z_MINB)
+// Reciprocal to ~1 ulp: MUFU.RCP64H seed (>= 20 bits) + two Newton steps.  The operands here are
+// pivot products |q| >= 1 of a diagonally dominant matrix -- never zero, subnormal or infinite.
+__device__ __forceinline__ double fast_rcp(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    return r;
+}
+
+// Neumann / Dirichlet in z.  One thread per real element of a plane; block of TH threads.
+//
+// Division-free sweeps.  Inside a block of CB rows starting at k0 the pivots are carried as the
+// ratio g_k = q_i / q_{i+1} (k = k0 + i) of the three-term recurrence
+//     q_{-1} = g_{k0-1},  q_0 = 1,  q_{i+1} = b_k q_i - q_{i-1}
+// and the eliminated right-hand side as y_i = x'_k q_{i+1}:
+//     y_i = r_k q_i - y_{i-1}                                   (y_{-1} = x'_{k0-1})
+// -- one dependent FMA per row on each chain instead of a dependent division.  The forward sweep
+// stores y_i and renormalises (one reciprocal) at the end of every block, where it also leaves the
+// checkpoint g_{k0-1} in shared memory; |q| grows by at most |b|^CB inside a block.  The backward
+// sweep recomputes the block's q_i bit-identically from the checkpoint and substitutes
+//     x_k = (y_i - q_i x_{k+1}) / q_{i+1},
+// whose reciprocals are off the dependency chain.
+//
+// Two-sided elimination.  T is persymmetric (same first and last diagonal), so eliminating upwards
+// from the last row produces the same pivots as eliminating downwards from the first.  Each thread
+// therefore runs both at once -- rows kk and nz-1-kk, kk = 0 .. ceil(nz/2)-1, share one pivot chain
+// and give two independent right-hand-side chains and twice the loads in flight -- couples the two
+// halves in the middle with a 2x2 solve, and substitutes outwards in both directions.  Half the
+// pivot arithmetic, and the same memory-level parallelism from half as many resident threads, which
+// keeps the forward sweep's output in L2 until the backward sweep re-reads it.
+template <int CB, bool FIRST>
+__device__ __forceinline__ void z_block_pivots(double (&qq)[CB + 1], double qm, double bint, double bend) {
+    qq[0] = 1.0;
+#pragma unroll
+    for (int i = 0; i < CB; ++i) {
+        const double bk = (FIRST && i == 0) ? bend : bint;
+        qq[i + 1] = fma(bk, qq[i], -qm);
+        qm = qq[i];
+    }
+}
+
+struct ZHalfState {
+    double g, xt, xb;          // normalised carries: pivot ratio, x' of the top chain, x' of the bottom chain
+    double qcap, qmcap, ycap;  // bottom chain's state at its last row (only when it ends before the top chain)
+};
+
+// rows kk = k0 .. k0+CB-1 of both halves.  m = rows of the top half, nb = rows of the bottom half.
+template <int CB, bool FIRST, bool RAGGED>
+__device__ __forceinline__ void z_forward_block(double *top, double *bot, ptrdiff_t plane, int k0, int m, int nb,
+                                                double bint, double bend, double scale, bool pin,
+                                                const ZPolicy &pol, ZHalfState &st) {
+    double rt[CB], rb[CB];
+#pragma unroll
+    for (int i = 0; i < CB; ++i) {
+        const int kk = k0 + i;
+        rt[i] = (!RAGGED || kk < m) ? ld_hint(top + kk * plane, pol.first) : 0.0;
+        rb[i] = (!RAGGED || kk < nb) ? ld_hint(bot - kk * plane, pol.first) : 0.0;
+    }
+    double qm = st.g, q = 1.0, yt = st.xt, yb = st.xb;
+#pragma unroll
+    for (int i = 0; i < CB; ++i) {
+        const int kk = k0 + i;
+        if (!RAGGED || kk < m) {
+            const double bk = (FIRST && i == 0) ? bend : bint;
+            yt = fma(rt[i] * scale, q, -yt);
+            if (!pin) st_hint(top + kk * plane, yt, pol.last);
+            if (!RAGGED || kk < nb) {
+                yb = fma(rb[i] * scale, q, -yb);
+                if (!pin) st_hint(bot - kk * plane, yb, pol.last);
+            }
+            const double qn = fma(bk, q, -qm);
+            qm = q;
+            q = qn;
+            if (RAGGED && kk == nb - 1) { st.qcap = q; st.qmcap = qm; st.ycap = yb; }
+        }
+    }
+    const double rq = fast_rcp(q);
+    st.g = qm * rq;
+    st.xt = yt * rq;
+    st.xb = yb * rq;
+}
+
+template <int CB, bool FIRST, bool RAGGED>
+__device__ __forceinline__ void z_backward_block(double *top, double *bot, ptrdiff_t plane, int k0, int m, int nb,
+                                                 double gprev, double bint, double bend, bool pin,
+                                                 const ZPolicy &pol, double &xt, double &xb) {
+    double qq[CB + 1], yt[CB], yb[CB];
+#pragma unroll
+    for (int i = 0; i < CB; ++i) {
+        const int kk = k0 + i;
+        yt[i] = (!RAGGED || kk < m) ? ld_hint(top + kk * plane, pol.first) : 0.0;
+        yb[i] = (!RAGGED || kk < nb) ? ld_hint(bot - kk * plane, pol.first) : 0.0;
+    }
+    z_block_pivots<CB, FIRST>(qq, gprev, bint, bend);
+#pragma unroll
+    for (int i = CB - 1; i >= 0; --i) {
+        const int kk = k0 + i;
+        if (!RAGGED || kk < m) {
+            const double rq = fast_rcp(qq[i + 1]);
+            const double c = qq[i] * rq;
+            xt = fma(-c, xt, yt[i] * rq);
+            if (!pin) st_hint(top + kk * plane, xt, pol.first);
+            if (!RAGGED || kk < nb) {
+                xb = fma(-c, xb, yb[i] * rq);
+                if (!pin) st_hint(bot - kk * plane, xb, pol.first);
+            }
+        }
+    }
+}
+
+template <int CB, int TH>
+__global__ void __launch_bounds__(TH, PP_Z_MINB)
 zsolve_thomas_kernel(double *w, ZParams p) {
+    extern __shared__ double ck[];                            // [nblk][TH] checkpoints g_{k0-1}
     const size_t plane = (size_t)p.nx * p.ny;
-    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t e = (size_t)blockIdx.x * TH + threadIdx.x;
     const bool live = e < plane;                              // dead threads run along (warp-wide zero-mode solve) but never store
     const int ix = live ? (int)(e % p.nx) : 0, j = live ? (int)(e / p.nx) : 0;
     const bool pin = !live || (p.singular && e == 0);
@@ -155,50 +270,50 @@ zsolve_thomas_kernel(double *w, ZParams p) {
     const double bint = -2.0 + s;
     const double bend = ((p.bcz == 1) ? -1.0 : -3.0) + s;
     const int nz = p.nz;
+    const int m = (nz + 1) / 2, nb = nz - m;                  // top rows [0, m), bottom rows nz-1-kk, kk in [0, nb)
+    const int nblk = (m + CB - 1) / CB;
     const double scale = p.scale;
-    double *col = w + (live ? e : 0);
+    const ptrdiff_t pl = (ptrdiff_t)plane;
+    double *top = w + (live ? e : 0);
+    double *bot = top + (ptrdiff_t)(nz - 1) * pl;
     const ZPolicy pol;
-    double ck[Z_MAX_CK];
+    double *myck = ck + threadIdx.x;
 
-    // forward sweep, in blocks of CB rows: batch the loads, then run the chain
-    double g = 0.0, xp = 0.0;
-    for (int k0 = 0; k0 < nz; k0 += CB) {
-        ck[k0 / CB] = g;
-        double r[CB];
-#pragma unroll
-        for (int i = 0; i < CB; ++i) r[i] = (k0 + i < nz) ? ld_hint(col + (size_t)(k0 + i) * plane, pol.first) : 0.0;
-#pragma unroll
-        for (int i = 0; i < CB; ++i) {
-            const int k = k0 + i;
-            if (k < nz) {
-                const double bk = (k == 0 || k == nz - 1) ? bend : bint;
-                g = 1.0 / (bk - g);
-                xp = (r[i] * scale - xp) * g;
-                if (!pin) st_hint(col + (size_t)k * plane, xp, pol.last);
-            }
+    // forward elimination from both ends
+    ZHalfState st = {0.0, 0.0, 0.0, 1.0, 0.0, 0.0};
+    for (int b = 0; b < nblk; ++b) {
+        const int k0 = b * CB;
+        myck[b * TH] = st.g;
+        const bool ragged = (k0 + CB > m) || (nb != m && k0 + CB >= nb);   // guards, and the bottom chain's last row
+        if (b == 0) {
+            if (ragged) z_forward_block<CB, true, true>(top, bot, pl, k0, m, nb, bint, bend, scale, pin, pol, st);
+            else        z_forward_block<CB, true, false>(top, bot, pl, k0, m, nb, bint, bend, scale, pin, pol, st);
+        } else {
+            if (ragged) z_forward_block<CB, false, true>(top, bot, pl, k0, m, nb, bint, bend, scale, pin, pol, st);
+            else        z_forward_block<CB, false, false>(top, bot, pl, k0, m, nb, bint, bend, scale, pin, pol, st);
         }
     }
-    // backward sweep
-    double x = xp;                                            // x_{nz-1} = x'_{nz-1}, already stored
-    for (int k0 = ((nz - 1) / CB) * CB; k0 >= 0; k0 -= CB) {
-        double gl[CB], r[CB];
-        double gg = ck[k0 / CB];
-#pragma unroll
-        for (int i = 0; i < CB; ++i) r[i] = (k0 + i < nz - 1) ? ld_hint(col + (size_t)(k0 + i) * plane, pol.first) : 0.0;
-#pragma unroll
-        for (int i = 0; i < CB; ++i) {
-            const int k = k0 + i;
-            const double bk = (k == 0 || k == nz - 1) ? bend : bint;
-            gg = 1.0 / (bk - gg);
-            gl[i] = gg;
-        }
-#pragma unroll
-        for (int i = CB - 1; i >= 0; --i) {
-            const int k = k0 + i;
-            if (k < nz - 1) {
-                x = r[i] - gl[i] * x;
-                if (!pin) st_hint(col + (size_t)k * plane, x, pol.first);
-            }
+    // couple the halves:  x_{m-1} + g_t x_m = x'_t,   x_m + g_b x_{m-1} = x'_b
+    double gb = st.g, xpb = st.xb;
+    if (nb != m) {                                            // odd nz: the bottom chain ended one row earlier
+        const double rqc = fast_rcp(st.qcap);
+        gb = st.qmcap * rqc;
+        xpb = st.ycap * rqc;
+    }
+    const double rden = 1.0 / (1.0 - st.g * gb);
+    double xt = (xpb - gb * st.xt) * rden;                    // x_m     : the row after the top half's last
+    double xb = (st.xt - st.g * xpb) * rden;                  // x_{m-1} : the row after the bottom half's last
+    // back substitution outwards
+    for (int b = nblk - 1; b >= 0; --b) {
+        const int k0 = b * CB;
+        const double gprev = myck[b * TH];
+        const bool ragged = (k0 + CB > m) || (nb != m && k0 + CB >= nb);   // guards, and the bottom chain's last row
+        if (b == 0) {
+            if (ragged) z_backward_block<CB, true, true>(top, bot, pl, k0, m, nb, gprev, bint, bend, pin, pol, xt, xb);
+            else        z_backward_block<CB, true, false>(top, bot, pl, k0, m, nb, gprev, bint, bend, pin, pol, xt, xb);
+        } else {
+            if (ragged) z_backward_block<CB, false, true>(top, bot, pl, k0, m, nb, gprev, bint, bend, pin, pol, xt, xb);
+            else        z_backward_block<CB, false, false>(top, bot, pl, k0, m, nb, gprev, bint, bend, pin, pol, xt, xb);
         }
     }
     // the warp that owns element 0 solves the singular line together (block 0, warp 0: all lanes alive)
