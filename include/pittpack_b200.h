@@ -107,6 +107,22 @@ size_t pp_plan_workspace_bytes(const pp_plan *plan);
 int pp_plan_set_profiling(pp_plan *plan, int enable);
 int pp_plan_last_kernel_ms(pp_plan *plan, float *ms_out);
 
+/*
+ * Which kernel solves the tridiagonal systems in z (PAPER.md:208-218 leaves the choice of
+ * tridiagonal algorithm open and offers several).  Both compute the same
+ * Thomas elimination of Algorithm 2 up to rounding order.
+ *   PP_Z_AUTO      : partitioned where it applies, two-sweep otherwise (the default).
+ *   PP_Z_SWEEP     : two-sweep Thomas, one thread per system, any nz; periodic z always uses it
+ *                    (Sherman-Morrison).
+ *   PP_Z_PARTITION : each system cut into segments of 32 or 64 rows held in registers and
+ *                    coupled through their interface unknowns (the reduction idea of CR-P,
+ *                    PAPER.md:250-258, across the threads of one CTA).  Needs Neumann or
+ *                    Dirichlet z and nz = 32 m or 64 m (m <= 8), 1024 or 2048; otherwise
+ *                    PP_ERR_UNSUPPORTED_SIZE and the plan is left unchanged.
+ */
+enum { PP_Z_AUTO = 0, PP_Z_SWEEP = 1, PP_Z_PARTITION = 2 };
+int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm);
+
 /* Static, NUL-terminated description of a status code. */
 const char *pp_strerror(int status);
 

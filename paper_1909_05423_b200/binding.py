@@ -21,8 +21,9 @@ KERNEL_NAMES = ("x_fwd", "y_fwd", "z_solve", "y_inv", "x_inv")
 
 EXPORTS = (
     "pp_plan_create", "pp_solve", "pp_solve_host", "pp_plan_destroy", "pp_plan_workspace_bytes",
-    "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_strerror", "pp_version",
+    "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_strerror", "pp_version",
 )
+PP_Z_AUTO, PP_Z_SWEEP, PP_Z_PARTITION = 0, 1, 2
 
 _lib = None
 
@@ -58,6 +59,8 @@ def lib() -> ctypes.CDLL:
     L.pp_plan_set_profiling.restype = i32
     L.pp_plan_last_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
     L.pp_plan_last_kernel_ms.restype = i32
+    L.pp_plan_set_z_algorithm.argtypes = [vp, i32]
+    L.pp_plan_set_z_algorithm.restype = i32
     L.pp_strerror.argtypes = [i32]
     L.pp_strerror.restype = ctypes.c_char_p
     L.pp_version.argtypes = []
@@ -102,6 +105,10 @@ def pp_plan_last_kernel_ms(plan):
     buf = (ctypes.c_float * PP_NUM_KERNELS)()
     st = lib().pp_plan_last_kernel_ms(ctypes.c_void_p(plan), buf)
     return st, [float(v) for v in buf]
+
+
+def pp_plan_set_z_algorithm(plan, algorithm):
+    return lib().pp_plan_set_z_algorithm(ctypes.c_void_p(plan), int(algorithm))
 
 
 def strerror(status: int) -> str:
@@ -178,6 +185,13 @@ class Plan:
         if st != PP_SUCCESS:
             raise PittPackError(st, "pp_plan_last_kernel_ms")
         return dict(zip(KERNEL_NAMES, ms))
+
+    def set_z_algorithm(self, algorithm):
+        """'auto' | 'sweep' | 'partition' (or a PP_Z_* value)."""
+        alg = {"auto": PP_Z_AUTO, "sweep": PP_Z_SWEEP, "partition": PP_Z_PARTITION}.get(algorithm, algorithm)
+        st = pp_plan_set_z_algorithm(self.handle, alg)
+        if st != PP_SUCCESS:
+            raise PittPackError(st, "pp_plan_set_z_algorithm")
 
     @property
     def workspace_bytes(self):

@@ -14,6 +14,7 @@
 #include "pp_xpass.cuh"
 #include "pp_ypass.cuh"
 #include "pp_zsolve.cuh"
+#include "pp_zpart.cuh"
 
 using namespace pp;
 
@@ -32,6 +33,7 @@ struct pp_plan {
     size_t bytes;
     int profiling;
     int have_times;
+    int z_algorithm;           // PP_Z_AUTO / PP_Z_SWEEP / PP_Z_PARTITION
     cudaEvent_t ev[PP_NUM_KERNELS + 1];
 };
 
@@ -177,7 +179,19 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
 #ifndef PP_Z_CB
 #define PP_Z_CB 16
 #endif
-    if (p->bcz != PP_BC_PERIODIC) {
+    const ZPartShape zs = (p->bcz != PP_BC_PERIODIC && p->z_algorithm != PP_Z_SWEEP) ? zpart_shape(p->nz) : ZPartShape{0, 0, 0};
+    if (zs.R) {
+        // partitioned, register-resident solve: one HBM read + one write per unknown (pp_zpart.cuh)
+        const size_t ds = zpart_smem_bytes(zs);
+        const unsigned grid = (unsigned)((plane + zs.L - 1) / zs.L);
+        if (zs.R == 32) {
+            if (int rc = set_smem(zsolve_part_kernel<32>, ds)) return rc;
+            zsolve_part_kernel<32><<<grid, zs.L * zs.S, ds, st>>>(w, zp, zs.S, zs.L);
+        } else {
+            if (int rc = set_smem(zsolve_part_kernel<64>, ds)) return rc;
+            zsolve_part_kernel<64><<<grid, zs.L * zs.S, ds, st>>>(w, zp, zs.S, zs.L);
+        }
+    } else if (p->bcz != PP_BC_PERIODIC) {
         // checkpoint table in shared memory: ceil(nz / CB) x TH doubles per CTA
 #define PP_ZT_LAUNCH(C, T)                                                                           \
         do {                                                                                         \
@@ -349,6 +363,15 @@ int pp_plan_set_profiling(pp_plan *plan, int enable) {
     if (!plan) return PP_ERR_NULL;
     plan->profiling = enable ? 1 : 0;
     plan->have_times = 0;
+    return PP_SUCCESS;
+}
+
+int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm) {
+    if (!plan) return PP_ERR_NULL;
+    if (algorithm != PP_Z_AUTO && algorithm != PP_Z_SWEEP && algorithm != PP_Z_PARTITION) return PP_ERR_INVALID_ARG;
+    if (algorithm == PP_Z_PARTITION && (plan->bcz == PP_BC_PERIODIC || zpart_shape(plan->nz).R == 0))
+        return PP_ERR_UNSUPPORTED_SIZE;
+    plan->z_algorithm = algorithm;
     return PP_SUCCESS;
 }
 

@@ -1,0 +1,233 @@
+// z-solve, register-resident partitioned variant: the same tridiagonal systems as pp_zsolve.cuh
+// (Algorithm 2), each read from HBM once and written once.
+//
+// The Thomas sweep of pp_zsolve.cuh touches every unknown twice (forward x', backward x) and
+// relies on the L2 to keep x' between the sweeps.  Here a z line of nz = R S rows is cut into S
+// segments of R rows; S threads own one system, each keeps its R right-hand sides in registers,
+// and the segments are coupled by the partition ("spike") form of the elimination -- the same
+// arithmetic the paper's CR-P reduction phase does across ranks, done across
+// the threads of one CTA:
+//
+//   segment block B (R x R, diagonal d_i, off-diagonals 1), neighbours xl = x_{a-1}, xr = x_{a+R}:
+//       x_loc = y - v xl - w xr,      y = B^-1 r_loc,  v = B^-1 e_0,  w = B^-1 e_{R-1}
+//   With the leading minors q_0 = 1, q_1 = d_0, q_{i+1} = d_i q_i - q_{i-1} (det B = q_R):
+//       Thomas pivots  g_i = q_i / q_{i+1}                      (g_k = 1/beta_k of Algorithm 1)
+//       w_i = (-1)^(R-1-i) q_i / q_R,   v_i = (-1)^i q_{R-1-i} / q_R  (Toeplitz block)
+//   so one table of q per system serves the pivots and both spikes.  Only two distinct blocks
+//   exist per system: the interior block (all d_i = b) and the first block (d_0 = b_end); the last
+//   block is the first one mirrored, and its owner simply holds its rows in reverse order.
+//
+//   The 2(S-1) interface unknowns (last row of segment J, first row of segment J+1) satisfy a
+//   block-tridiagonal system with 2x2 blocks.  Its matrix depends on the mode only, so it is
+//   factored (the divisions) while the loads are still in flight; the right-hand-side part is a
+//   short FMA chain run by one thread per system through shared memory.  Every segment then
+//   applies  x_i = y_i - v_i xl - w_i xr  and stores.
+//
+// Thread mapping: CTA = L lanes x S segments; lane l owns system blockIdx.x L + l (consecutive x:
+// every row access of a segment is one coalesced L*8-byte run), thread (l, j) owns rows
+// [j R, (j+1) R).  All R loads of a thread are issued before anything else, so a resident CTA has
+// its whole tile (L nz doubles) in flight.
+//
+// Neumann / Dirichlet z only (periodic z keeps the Sherman-Morrison kernel); nz must
+// be R S with R in {32, 64}; other sizes keep the two-sweep kernel.  The singular (0,0) line is
+// handled by zero_mode_line exactly as there.
+#pragma once
+#include "pp_zsolve.cuh"
+
+namespace pp {
+
+struct ZPartShape {
+    int R, S, L;              // rows per thread, segments per system, systems per CTA
+};
+
+// which (R, S, L) serves this nz; R == 0: not supported by the partitioned kernel
+#ifndef PP_ZP_MAXT
+#define PP_ZP_MAXT 256    // threads per CTA (L S) never exceeds this
+#define PP_ZP_MINB 2      // resident CTAs per SM the R = 32 kernel is compiled for (R = 64: half)
+#endif
+#ifndef PP_ZP_L
+#define PP_ZP_L 32        // systems per CTA when S <= 8
+#endif
+inline ZPartShape zpart_shape(int nz) {
+    if (nz % 32 == 0 && nz / 32 <= 8) return {32, nz / 32, PP_ZP_L};
+    if (nz % 64 == 0 && nz / 64 <= 8) return {64, nz / 64, PP_ZP_L};
+    if (nz == 1024) return {64, 16, 16};
+    if (nz == 2048) return {64, 32, 8};
+    return {0, 0, 0};
+}
+
+// dynamic shared memory of one CTA, in doubles:
+//   Q [2][R+1][L]   leading minors of the first (0) and interior (1) block
+//   G [2][R][L]     pivots g_i
+//   YF, YL [S][L]   first / last row of every segment's local solution; overwritten by the
+//                   interface solution (XL[j] = x just above segment j, XR[j] = x just below it)
+//   F [6][S][L]     factored interface matrix (right-hand-side independent): vL, vF, D, A, sc, sa
+//   PC, PA [S][L]   right-hand-side part of the interface elimination
+inline size_t zpart_smem_bytes(const ZPartShape &z) {
+    return sizeof(double) * (size_t)z.L * (2 * (z.R + 1) + 2 * z.R + 10 * z.S);
+}
+
+// keeps the compiler from hoisting a whole unrolled loop's shared-memory loads above it (which
+// costs more registers than the cap allows and ends in local-memory spills)
+__device__ __forceinline__ void zp_sched_fence() { asm volatile("" ::: "memory"); }
+
+// leading minors of one block: q_0 = 1, q_1 = d_0, q_{i+1} = d_i q_i - q_{i-1}; returns q_{R-1}, q_R
+// and, if TABLES, stores q_i to q[i L] and the pivots g_i = q_i / q_{i+1} to g[i L]
+template <int R, bool TABLES>
+__device__ __forceinline__ void zp_minors(double d0, double dint, double dlast, double *q, double *g, int L,
+                                          double &qRm1, double &qR) {
+    double qm = 1.0, qc = d0;
+    if (TABLES) { q[0] = qm; q[L] = qc; g[0] = fast_rcp(qc); }
+#pragma unroll
+    for (int i = 1; i < R; ++i) {
+        const double qn = fma((i == R - 1) ? dlast : dint, qc, -qm);
+        qm = qc;
+        qc = qn;
+        if (TABLES) { q[(i + 1) * L] = qn; g[i * L] = qm * fast_rcp(qn); }
+    }
+    qRm1 = qm;
+    qR = qc;
+}
+
+template <int R>
+__global__ void __launch_bounds__(PP_ZP_MAXT, (R == 32) ? PP_ZP_MINB : PP_ZP_MINB / 2)
+zsolve_part_kernel(double *w, ZParams p, int S, int L) {
+    static_assert(R % 2 == 0, "the spike signs below assume an even segment length");
+    extern __shared__ double zsm[];
+    double *Q = zsm;                                  // [2][R+1][L]
+    double *G = Q + 2 * (R + 1) * L;                  // [2][R][L]
+    double *YF = G + 2 * R * L;                       // [S][L], later XL
+    double *YL = YF + S * L;                          // [S][L], later XR
+    double *F = YL + S * L;                           // [6][S][L]
+    double *PC = F + 6 * S * L, *PA = PC + S * L;
+    const int SL = S * L;
+
+    const int l = threadIdx.x % L, j = threadIdx.x / L;
+    const size_t plane = (size_t)p.nx * p.ny;
+    const size_t e = (size_t)blockIdx.x * L + l;
+    const bool live = e < plane;
+    const bool pin = !live || (p.singular && e == 0);       // pinned line: computed with a placeholder, never stored
+    const bool mirror = (S > 1) && (j == S - 1);              // last segment: rows held in reverse order
+    const int c = (j == 0 || j == S - 1) ? 0 : 1;             // which block: first (and mirrored last) / interior
+    // row i of the segment lives at row0 + i * step (the mirrored segment walks upwards)
+    const ptrdiff_t step = mirror ? -(ptrdiff_t)plane : (ptrdiff_t)plane;
+    double *row0 = w + (live ? e : 0) + ((size_t)j * R + (mirror ? R - 1 : 0)) * plane;
+
+    // every right-hand side of the segment, in flight at once
+    double y[R];
+#pragma unroll
+    for (int i = 0; i < R; ++i) y[i] = __ldcs(row0 + i * step);
+
+    // While the loads fly: segment 0's thread tabulates the first block, segment 1's the interior
+    // block, segment 2's (segment 1's when S = 2) factors the interface matrix.
+    const int jfac = (S >= 3) ? 2 : 1;
+    if (j <= jfac) {
+        const int ix = live ? (int)(e % p.nx) : 0, jy = live ? (int)(e / p.nx) : 0;
+        const double s = pin ? -1.0 : (p.sx[ix] + p.sy[jy]);
+        const double bint = -2.0 + s;
+        const double bend = ((p.bcz == 1) ? -1.0 : -3.0) + s;
+        double qa, qb;
+        if (j == 0) {
+            zp_minors<R, true>(bend, bint, (S == 1) ? bend : bint, Q + l, G + l, L, qa, qb);
+        } else if (j == 1 && S >= 3) {
+            zp_minors<R, true>(bint, bint, bint, Q + (R + 1) * L + l, G + R * L + l, L, qa, qb);
+        } else {
+            // interface system, unknowns a_J = last row of segment J, c_J = first row of segment J+1:
+            //   a_J + vL_J a_{J-1} + wL_J c_J         = yL_J
+            //   c_J + vF_{J+1} a_J + wF_{J+1} c_{J+1} = yF_{J+1}
+            // end blocks:      wL = vF = q_{R-1}/q_R =: a0,  no outward coupling
+            // interior blocks: wL = vF = q_{R-1}/q_R =: a1,  vL = wF = (-1)^(R-1)/q_R =: b1
+            // block Thomas: a_J = pa_J - sa_J c_{J+1},  c_J = pc_J - sc_J c_{J+1};  A, D, sc, sa are
+            // right-hand-side independent and computed here.
+            zp_minors<R, false>(bend, bint, bint, nullptr, nullptr, L, qa, qb);
+            const double a0 = qa / qb;
+            double a1 = 0.0, b1 = 0.0;
+            if (S >= 3) {
+                zp_minors<R, false>(bint, bint, bint, nullptr, nullptr, L, qa, qb);
+                a1 = qa / qb;
+                b1 = -1.0 / qb;
+            }
+            double sa = 0.0;
+            for (int J = 0; J < S - 1; ++J) {
+                const double wL = (J == 0) ? a0 : a1, vL = (J == 0) ? 0.0 : b1;
+                const double vF = (J + 1 == S - 1) ? a0 : a1, wF = (J + 1 == S - 1) ? 0.0 : b1;
+                const double A = wL - vL * sa;
+                const double D = 1.0 / (1.0 - vF * A);
+                const double sc = D * wF;
+                sa = -A * sc;
+                double *f = F + J * L + l;
+                f[0] = vL; f[SL] = vF; f[2 * SL] = D; f[3 * SL] = A; f[4 * SL] = sc; f[5 * SL] = sa;
+            }
+        }
+    }
+    __syncthreads();
+
+    // local solve  y = B^-1 (scale r)  in registers (Algorithm 1 with the tabulated pivots)
+    {
+        const double *g = G + c * R * L + l;
+        const double scale = p.scale;
+        y[0] = y[0] * scale * g[0];
+#pragma unroll
+        for (int i = 1; i < R; ++i) {
+            y[i] = fma(y[i], scale, -y[i - 1]) * g[i * L];
+            if (i % 8 == 7) zp_sched_fence();
+        }
+#pragma unroll
+        for (int i = R - 2; i >= 0; --i) {
+            y[i] = fma(-g[i * L], y[i + 1], y[i]);
+            if (i % 8 == 0) zp_sched_fence();
+        }
+    }
+
+    if (S > 1) {
+        YF[j * L + l] = mirror ? y[R - 1] : y[0];
+        YL[j * L + l] = mirror ? y[0] : y[R - 1];
+        __syncthreads();
+        if (j == 0) {                                   // right-hand-side part of the interface elimination
+            double pa = 0.0;
+            for (int J = 0; J < S - 1; ++J) {
+                const double *f = F + J * L + l;
+                const double Ya = fma(-f[0], pa, YL[J * L + l]);
+                const double pc = f[2 * SL] * fma(-f[SL], Ya, YF[(J + 1) * L + l]);
+                pa = fma(-f[3 * SL], pc, Ya);
+                PC[J * L + l] = pc;
+                PA[J * L + l] = pa;
+            }
+            double cn = 0.0;
+            for (int J = S - 2; J >= 0; --J) {
+                const double *f = F + J * L + l;
+                const double cv = fma(-f[4 * SL], cn, PC[J * L + l]);
+                const double av = fma(-f[5 * SL], cn, PA[J * L + l]);
+                YL[J * L + l] = cv;                  // XR of segment J   = first row of segment J+1
+                YF[(J + 1) * L + l] = av;            // XL of segment J+1 = last row of segment J
+                cn = cv;
+            }
+        }
+        __syncthreads();
+        const double *qc = Q + c * (R + 1) * L + l;
+        const double xlg = (j >= 1) ? YF[j * L + l] : 0.0;
+        const double xrg = (j <= S - 2) ? YL[j * L + l] : 0.0;
+        const double rq = 1.0 / qc[R * L];
+        const double XL = (c == 0) ? 0.0 : xlg * rq;
+        const double XR = ((c == 0 && mirror) ? xlg : xrg) * rq;
+        // x_i = y_i - v_i xl - w_i xr = y_i - (-1)^i (q_{R-1-i} XL - q_i XR)
+#pragma unroll
+        for (int i = 0; i < R; i += 2) {
+            y[i] = fma(qc[i * L], XR, fma(-qc[(R - 1 - i) * L], XL, y[i]));
+            y[i + 1] = fma(-qc[(i + 1) * L], XR, fma(qc[(R - 2 - i) * L], XL, y[i + 1]));
+            if (i % 8 == 6) zp_sched_fence();
+        }
+    }
+    if (!pin) {
+        // recompute the row addresses instead of keeping the R load addresses alive (registers)
+        double *out0 = row0;
+        ptrdiff_t ostep = step;
+        asm volatile("" : "+l"(out0), "+l"(ostep));
+#pragma unroll
+        for (int i = 0; i < R; ++i) __stcs(out0 + i * ostep, y[i]);
+    }
+    // the warp that owns element 0 solves the singular line together (its line was never stored above)
+    if (p.singular && blockIdx.x == 0 && threadIdx.x < 32) zero_mode_line(w, plane, p.nz, p.bcz, p.scale, p.zero_scratch);
+}
+
+}  // namespace pp
