@@ -63,8 +63,9 @@ inline ZPartShape zpart_shape(int nz) {
 //                   interface solution (XL[j] = x just above segment j, XR[j] = x just below it)
 //   F [6][S][L]     factored interface matrix (right-hand-side independent): vL, vF, D, A, sc, sa
 //   PC, PA [S][L]   right-hand-side part of the interface elimination
+//   RQ [2][L]       1 / q_R of the two blocks
 inline size_t zpart_smem_bytes(const ZPartShape &z) {
-    return sizeof(double) * (size_t)z.L * (2 * (z.R + 1) + 2 * z.R + 10 * z.S);
+    return sizeof(double) * (size_t)z.L * (2 * (z.R + 1) + 2 * z.R + 10 * z.S + 2);
 }
 
 // keeps the compiler from hoisting a whole unrolled loop's shared-memory loads above it (which
@@ -100,6 +101,7 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L) {
     double *YL = YF + S * L;                          // [S][L], later XR
     double *F = YL + S * L;                           // [6][S][L]
     double *PC = F + 6 * S * L, *PA = PC + S * L;
+    double *RQ = PA + S * L;                          // [2][L]
     const int SL = S * L;
 
     const int l = threadIdx.x % L, j = threadIdx.x / L;
@@ -129,9 +131,12 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L) {
         double qa, qb;
         if (j == 0) {
             zp_minors<R, true>(bend, bint, (S == 1) ? bend : bint, Q + l, G + l, L, qa, qb);
-        } else if (j == 1 && S >= 3) {
+            RQ[l] = fast_rcp(qb);
+        } else if (j == 1) {
             zp_minors<R, true>(bint, bint, bint, Q + (R + 1) * L + l, G + R * L + l, L, qa, qb);
-        } else {
+            RQ[L + l] = fast_rcp(qb);
+        }
+        if (j == jfac) {
             // interface system, unknowns a_J = last row of segment J, c_J = first row of segment J+1:
             //   a_J + vL_J a_{J-1} + wL_J c_J         = yL_J
             //   c_J + vF_{J+1} a_J + wF_{J+1} c_{J+1} = yF_{J+1}
@@ -139,20 +144,23 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L) {
             // interior blocks: wL = vF = q_{R-1}/q_R =: a1,  vL = wF = (-1)^(R-1)/q_R =: b1
             // block Thomas: a_J = pa_J - sa_J c_{J+1},  c_J = pc_J - sc_J c_{J+1};  A, D, sc, sa are
             // right-hand-side independent and computed here.
-            zp_minors<R, false>(bend, bint, bint, nullptr, nullptr, L, qa, qb);
-            const double a0 = qa / qb;
-            double a1 = 0.0, b1 = 0.0;
-            if (S >= 3) {
-                zp_minors<R, false>(bint, bint, bint, nullptr, nullptr, L, qa, qb);
-                a1 = qa / qb;
-                b1 = -1.0 / qb;
+            // (both blocks' minors again, interleaved in one loop: two independent FMA chains)
+            double em = 1.0, ec = bend, im = 1.0, ic = bint;
+#pragma unroll
+            for (int i = 1; i < R; ++i) {
+                const double en = fma(bint, ec, -em), in = fma(bint, ic, -im);
+                em = ec; ec = en;
+                im = ic; ic = in;
             }
+            const double rqe = fast_rcp(ec), rqi = fast_rcp(ic);
+            const double a0 = em * rqe;
+            const double a1 = (S >= 3) ? im * rqi : 0.0, b1 = (S >= 3) ? -rqi : 0.0;
             double sa = 0.0;
             for (int J = 0; J < S - 1; ++J) {
                 const double wL = (J == 0) ? a0 : a1, vL = (J == 0) ? 0.0 : b1;
                 const double vF = (J + 1 == S - 1) ? a0 : a1, wF = (J + 1 == S - 1) ? 0.0 : b1;
                 const double A = wL - vL * sa;
-                const double D = 1.0 / (1.0 - vF * A);
+                const double D = fast_rcp(fma(-vF, A, 1.0));
                 const double sc = D * wF;
                 sa = -A * sc;
                 double *f = F + J * L + l;
@@ -162,20 +170,34 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L) {
     }
     __syncthreads();
 
-    // local solve  y = B^-1 (scale r)  in registers (Algorithm 1 with the tabulated pivots)
+    // local solve  y = B^-1 (scale r)  in registers: Algorithm 1 with the tabulated pivots, run from
+    // both ends of the segment at once (rows k and R-1-k; two independent dependency chains of half
+    // the length).  Eliminating upwards from the far end of a block meets a pure Toeplitz diagonal,
+    // i.e. the interior block's pivots -- or, with a single segment, the first block's again.
     {
-        const double *g = G + c * R * L + l;
+        constexpr int M = R / 2;
+        const double *gt = G + c * R * L + l;
+        const double *gb = G + ((S == 1) ? 0 : R * L) + l;
         const double scale = p.scale;
-        y[0] = y[0] * scale * g[0];
+        y[0] = y[0] * scale * gt[0];
+        y[R - 1] = y[R - 1] * scale * gb[0];
 #pragma unroll
-        for (int i = 1; i < R; ++i) {
-            y[i] = fma(y[i], scale, -y[i - 1]) * g[i * L];
-            if (i % 8 == 7) zp_sched_fence();
+        for (int k = 1; k < M; ++k) {
+            y[k] = fma(y[k], scale, -y[k - 1]) * gt[k * L];
+            y[R - 1 - k] = fma(y[R - 1 - k], scale, -y[R - k]) * gb[k * L];
+            if (k % 4 == 3) zp_sched_fence();
         }
+        // couple the halves:  x_{M-1} + gt x_M = y_{M-1},   x_M + gb x_{M-1} = y_M
+        const double gtm = gt[(M - 1) * L], gbm = gb[(M - 1) * L];
+        const double rden = fast_rcp(fma(-gtm, gbm, 1.0));
+        const double xa = fma(-gtm, y[M], y[M - 1]) * rden, xb = fma(-gbm, y[M - 1], y[M]) * rden;
+        y[M - 1] = xa;
+        y[M] = xb;
 #pragma unroll
-        for (int i = R - 2; i >= 0; --i) {
-            y[i] = fma(-g[i * L], y[i + 1], y[i]);
-            if (i % 8 == 0) zp_sched_fence();
+        for (int k = M - 2; k >= 0; --k) {
+            y[k] = fma(-gt[k * L], y[k + 1], y[k]);
+            y[R - 1 - k] = fma(-gb[k * L], y[R - 2 - k], y[R - 1 - k]);
+            if (k % 4 == 0) zp_sched_fence();
         }
     }
 
@@ -184,30 +206,42 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L) {
         YL[j * L + l] = mirror ? y[0] : y[R - 1];
         __syncthreads();
         if (j == 0) {                                   // right-hand-side part of the interface elimination
+            // (the next step's coefficients are fetched before the current step's FMA chain)
+            const double *f = F + l;
+            double vL = f[0], vF = f[SL], D = f[2 * SL], A = f[3 * SL], yl = YL[l], yf = YF[L + l];
             double pa = 0.0;
             for (int J = 0; J < S - 1; ++J) {
-                const double *f = F + J * L + l;
-                const double Ya = fma(-f[0], pa, YL[J * L + l]);
-                const double pc = f[2 * SL] * fma(-f[SL], Ya, YF[(J + 1) * L + l]);
-                pa = fma(-f[3 * SL], pc, Ya);
+                const int Jn = (J + 1 < S - 1) ? J + 1 : J;
+                const double *fn = F + Jn * L + l;
+                const double nvL = fn[0], nvF = fn[SL], nD = fn[2 * SL], nA = fn[3 * SL];
+                const double nyl = YL[Jn * L + l], nyf = YF[(Jn + 1) * L + l];
+                const double Ya = fma(-vL, pa, yl);
+                const double pc = D * fma(-vF, Ya, yf);
+                pa = fma(-A, pc, Ya);
                 PC[J * L + l] = pc;
                 PA[J * L + l] = pa;
+                vL = nvL; vF = nvF; D = nD; A = nA; yl = nyl; yf = nyf;
             }
+            f = F + (S - 2) * L + l;
+            double sc = f[4 * SL], sa = f[5 * SL], pc = PC[(S - 2) * L + l], pav = PA[(S - 2) * L + l];
             double cn = 0.0;
             for (int J = S - 2; J >= 0; --J) {
-                const double *f = F + J * L + l;
-                const double cv = fma(-f[4 * SL], cn, PC[J * L + l]);
-                const double av = fma(-f[5 * SL], cn, PA[J * L + l]);
+                const int Jn = (J > 0) ? J - 1 : 0;
+                const double *fn = F + Jn * L + l;
+                const double nsc = fn[4 * SL], nsa = fn[5 * SL], npc = PC[Jn * L + l], npa = PA[Jn * L + l];
+                const double cv = fma(-sc, cn, pc);
+                const double av = fma(-sa, cn, pav);
                 YL[J * L + l] = cv;                  // XR of segment J   = first row of segment J+1
                 YF[(J + 1) * L + l] = av;            // XL of segment J+1 = last row of segment J
                 cn = cv;
+                sc = nsc; sa = nsa; pc = npc; pav = npa;
             }
         }
         __syncthreads();
         const double *qc = Q + c * (R + 1) * L + l;
         const double xlg = (j >= 1) ? YF[j * L + l] : 0.0;
         const double xrg = (j <= S - 2) ? YL[j * L + l] : 0.0;
-        const double rq = 1.0 / qc[R * L];
+        const double rq = RQ[c * L + l];
         const double XL = (c == 0) ? 0.0 : xlg * rq;
         const double XR = ((c == 0 && mirror) ? xlg : xrg) * rq;
         // x_i = y_i - v_i xl - w_i xr = y_i - (-1)^i (q_{R-1-i} XL - q_i XR)
