@@ -61,7 +61,7 @@ inline ZPartShape zpart_shape(int nz) {
 //   G [2][R][L]     pivots g_i
 //   YF, YL [S][L]   first / last row of every segment's local solution; overwritten by the
 //                   interface solution (XL[j] = x just above segment j, XR[j] = x just below it)
-//   F [6][S][L]     factored interface matrix (right-hand-side independent): vL, vF, D, A, sc, sa
+//   F [6][S][L]     factored interface matrix (right-hand-side independent): vL, vF, D, A D, sc, sa
 //   PC, PA [S][L]   right-hand-side part of the interface elimination
 //   RQ [2][L]       1 / q_R of the two blocks
 inline size_t zpart_smem_bytes(const ZPartShape &z) {
@@ -115,17 +115,18 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L) {
     const ptrdiff_t step = mirror ? -(ptrdiff_t)plane : (ptrdiff_t)plane;
     double *row0 = w + (live ? e : 0) + ((size_t)j * R + (mirror ? R - 1 : 0)) * plane;
 
-    // every right-hand side of the segment, in flight at once
+    // the mode's shift first (the tabulating threads start from it), then every right-hand side of
+    // the segment, in flight at once
+    const int jfac = (S >= 3) ? 2 : 1;
+    double s = -1.0;
+    if (j <= jfac && !pin) s = __ldg(p.sx + (int)(e % p.nx)) + __ldg(p.sy + (int)(e / p.nx));
     double y[R];
 #pragma unroll
     for (int i = 0; i < R; ++i) y[i] = __ldcs(row0 + i * step);
 
     // While the loads fly: segment 0's thread tabulates the first block, segment 1's the interior
     // block, segment 2's (segment 1's when S = 2) factors the interface matrix.
-    const int jfac = (S >= 3) ? 2 : 1;
     if (j <= jfac) {
-        const int ix = live ? (int)(e % p.nx) : 0, jy = live ? (int)(e / p.nx) : 0;
-        const double s = pin ? -1.0 : (p.sx[ix] + p.sy[jy]);
         const double bint = -2.0 + s;
         const double bend = ((p.bcz == 1) ? -1.0 : -3.0) + s;
         double qa, qb;
@@ -142,8 +143,9 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L) {
             //   c_J + vF_{J+1} a_J + wF_{J+1} c_{J+1} = yF_{J+1}
             // end blocks:      wL = vF = q_{R-1}/q_R =: a0,  no outward coupling
             // interior blocks: wL = vF = q_{R-1}/q_R =: a1,  vL = wF = (-1)^(R-1)/q_R =: b1
-            // block Thomas: a_J = pa_J - sa_J c_{J+1},  c_J = pc_J - sc_J c_{J+1};  A, D, sc, sa are
-            // right-hand-side independent and computed here.
+            // block Thomas: with A_J = wL_J - vL_J sa_{J-1}, D_J = 1 / (1 - vF_{J+1} A_J),
+            //   c_J = pc_J - sc_J c_{J+1},  a_J = pa_J - sa_J c_{J+1},  sc_J = D_J wF_{J+1},  sa_J = -A_J sc_J;
+            // A, D, sc, sa are right-hand-side independent and computed here.
             // (both blocks' minors again, interleaved in one loop: two independent FMA chains)
             double em = 1.0, ec = bend, im = 1.0, ic = bint;
 #pragma unroll
@@ -155,16 +157,21 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L) {
             const double rqe = fast_rcp(ec), rqi = fast_rcp(ic);
             const double a0 = em * rqe;
             const double a1 = (S >= 3) ? im * rqi : 0.0, b1 = (S >= 3) ? -rqi : 0.0;
-            double sa = 0.0;
+            // A_J obeys the Moebius recurrence A_0 = a0, A_J = a1 + b1^2 A_{J-1} / (1 - a1 A_{J-1}); carried
+            // as the ratio N_J / M_J it is two FMAs per step, and the reciprocals leave the dependency chain:
+            //   D_J = M_J / (M_J - vF_J N_J),   (A D)_J = N_J / (M_J - vF_J N_J)
+            const double k1 = fma(b1, b1, -a1 * a1);
+            double N = a0, M = 1.0;
             for (int J = 0; J < S - 1; ++J) {
-                const double wL = (J == 0) ? a0 : a1, vL = (J == 0) ? 0.0 : b1;
+                const double vL = (J == 0) ? 0.0 : b1;
                 const double vF = (J + 1 == S - 1) ? a0 : a1, wF = (J + 1 == S - 1) ? 0.0 : b1;
-                const double A = wL - vL * sa;
-                const double D = fast_rcp(fma(-vF, A, 1.0));
-                const double sc = D * wF;
-                sa = -A * sc;
+                const double r = fast_rcp(fma(-vF, N, M));
+                const double D = M * r, AD = N * r;
                 double *f = F + J * L + l;
-                f[0] = vL; f[SL] = vF; f[2 * SL] = D; f[3 * SL] = A; f[4 * SL] = sc; f[5 * SL] = sa;
+                f[0] = vL; f[SL] = vF; f[2 * SL] = D; f[3 * SL] = AD; f[4 * SL] = D * wF; f[5 * SL] = -AD * wF;
+                const double Nn = fma(k1, N, a1 * M), Mn = fma(-a1, N, M);
+                N = Nn;
+                M = Mn;
             }
         }
     }
@@ -216,8 +223,9 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L) {
                 const double nvL = fn[0], nvF = fn[SL], nD = fn[2 * SL], nA = fn[3 * SL];
                 const double nyl = YL[Jn * L + l], nyf = YF[(Jn + 1) * L + l];
                 const double Ya = fma(-vL, pa, yl);
-                const double pc = D * fma(-vF, Ya, yf);
-                pa = fma(-A, pc, Ya);
+                const double t = fma(-vF, Ya, yf);
+                const double pc = D * t;
+                pa = fma(-A, t, Ya);                 // A holds (A D)_J
                 PC[J * L + l] = pc;
                 PA[J * L + l] = pa;
                 vL = nvL; vF = nvF; D = nD; A = nA; yl = nyl; yf = nyf;
