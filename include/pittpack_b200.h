@@ -123,6 +123,18 @@ int pp_plan_last_kernel_ms(pp_plan *plan, float *ms_out);
 enum { PP_Z_AUTO = 0, PP_Z_SWEEP = 1, PP_Z_PARTITION = 2 };
 int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm);
 
+/*
+ * Plane-wise fusion of the x and y passes.  The 2-D transform of one xy plane is independent of
+ * every other plane.  With fusion enabled the x tiles and y tiles of a plane are
+ * tasks of ONE persistent kernel, ordered so that a plane's intermediate spectrum stays in the L2
+ * cache between its x and y pass: pp_solve then launches 3 kernels (x+y forward, z solve, y+x
+ * inverse) and HBM sees 48 instead of 80 bytes per point.  Results are bit-identical to the
+ * unfused path.  Needs nx == ny in {128, 256, 512, 1024}; otherwise PP_ERR_UNSUPPORTED_SIZE and the
+ * plan is left unchanged.  With fusion on, pp_plan_last_kernel_ms reports the fused kernels' times
+ * in the PP_K_XFWD and PP_K_XINV slots and 0 for PP_K_YFWD / PP_K_YINV.
+ */
+int pp_plan_set_xy_fusion(pp_plan *plan, int enable);
+
 /* Static, NUL-terminated description of a status code. */
 const char *pp_strerror(int status);
 

@@ -21,7 +21,7 @@ KERNEL_NAMES = ("x_fwd", "y_fwd", "z_solve", "y_inv", "x_inv")
 
 EXPORTS = (
     "pp_plan_create", "pp_solve", "pp_solve_host", "pp_plan_destroy", "pp_plan_workspace_bytes",
-    "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_strerror", "pp_version",
+    "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_plan_set_xy_fusion", "pp_strerror", "pp_version",
 )
 PP_Z_AUTO, PP_Z_SWEEP, PP_Z_PARTITION = 0, 1, 2
 
@@ -61,6 +61,8 @@ def lib() -> ctypes.CDLL:
     L.pp_plan_last_kernel_ms.restype = i32
     L.pp_plan_set_z_algorithm.argtypes = [vp, i32]
     L.pp_plan_set_z_algorithm.restype = i32
+    L.pp_plan_set_xy_fusion.argtypes = [vp, i32]
+    L.pp_plan_set_xy_fusion.restype = i32
     L.pp_strerror.argtypes = [i32]
     L.pp_strerror.restype = ctypes.c_char_p
     L.pp_version.argtypes = []
@@ -109,6 +111,10 @@ def pp_plan_last_kernel_ms(plan):
 
 def pp_plan_set_z_algorithm(plan, algorithm):
     return lib().pp_plan_set_z_algorithm(ctypes.c_void_p(plan), int(algorithm))
+
+
+def pp_plan_set_xy_fusion(plan, enable):
+    return lib().pp_plan_set_xy_fusion(ctypes.c_void_p(plan), int(bool(enable)))
 
 
 def strerror(status: int) -> str:
@@ -192,6 +198,11 @@ class Plan:
         st = pp_plan_set_z_algorithm(self.handle, alg)
         if st != PP_SUCCESS:
             raise PittPackError(st, "pp_plan_set_z_algorithm")
+
+    def set_xy_fusion(self, enable: bool):
+        st = pp_plan_set_xy_fusion(self.handle, enable)
+        if st != PP_SUCCESS:
+            raise PittPackError(st, "pp_plan_set_xy_fusion")
 
     @property
     def workspace_bytes(self):

@@ -15,6 +15,7 @@
 #include "pp_ypass.cuh"
 #include "pp_zsolve.cuh"
 #include "pp_zpart.cuh"
+#include "pp_fused.cuh"
 
 using namespace pp;
 
@@ -23,6 +24,7 @@ struct pp_plan {
     double dx, dy, dz;
     int bcx, bcy, bcz;
     int device;
+    int num_sms;
     int singular;
     double scale;
     double2 *tw_x, *tw_y;      // per-stage FFT twiddle tables (pp_fft.cuh, tw_stage_offset)
@@ -34,6 +36,8 @@ struct pp_plan {
     int profiling;
     int have_times;
     int z_algorithm;           // PP_Z_AUTO / PP_Z_SWEEP / PP_Z_PARTITION
+    int xy_fusion;             // 1: x and y passes of a plane run as tasks of one kernel (pp_fused.cuh)
+    int *fuse_sync;            // [1 + nz] ticket + per-plane completion counters
     cudaEvent_t ev[PP_NUM_KERNELS + 1];
 };
 
@@ -164,6 +168,53 @@ int run_y(const pp_plan *p, bool fwd, double *w, cudaStream_t st) {
 #undef CALL_Y
 }
 
+// nx == ny in {128, 256, 512, 1024}: the sizes the fused x+y kernel is instantiated for
+bool fusion_supported(int nx, int ny) { return nx == ny && nx >= 128 && nx <= 1024; }
+
+#ifndef PP_FUSE_LAG
+#define PP_FUSE_LAG 0          // 0: derived from the number of resident CTAs
+#endif
+
+template <int N, bool FWD_DIR>
+int launch_fused(const pp_plan *p, const double *in, double *u, cudaStream_t st) {
+    using Y = YCfg<N>;
+    constexpr int TX = Y::THREADS / FftCfg<N>::P;
+    auto kernel = xy_fused_kernel<N, FWD_DIR>;
+    if (int rc = set_smem(kernel, Y::SMEM)) return rc;
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, Y::THREADS, Y::SMEM) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError();
+        return PP_ERR_CUDA;
+    }
+    FusedParams fp;
+    fp.nz = p->nz; fp.nxh = p->nx / 2;
+    fp.pairs_per_plane = p->ny / 2;
+    const int xt = (int)((fp.pairs_per_plane + TX - 1) / TX), yt = (fp.nxh + Y::T - 1) / Y::T;
+    fp.na = FWD_DIR ? xt : yt;
+    fp.nb = FWD_DIR ? yt : xt;
+    const long long resident = (long long)p->num_sms * per_sm;
+    long long lag = PP_FUSE_LAG ? PP_FUSE_LAG : (5 * resident / (4 * (fp.na + fp.nb)) + 2);
+    fp.lag = (int)(lag < 1 ? 1 : (lag > p->nz ? p->nz : lag));
+    fp.bcx = p->bcx; fp.bcy = p->bcy;
+    fp.complex_cols = (p->bcx == PP_BC_PERIODIC && p->bcy == PP_BC_PERIODIC) ? 1 : 0;
+    fp.sync = p->fuse_sync;
+    if (cudaMemsetAsync(p->fuse_sync, 0, sizeof(int) * (size_t)(p->nz + 1), st) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    const long long total = (long long)p->nz * (fp.na + fp.nb);
+    const unsigned grid = (unsigned)(total < resident ? total : resident);
+    kernel<<<grid, Y::THREADS, Y::SMEM, st>>>(in, u, fp, p->tw_x, p->ptw_x, p->tw_y, p->ptw_y);
+    return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
+}
+
+int run_fused(const pp_plan *p, bool fwd, const double *in, double *u, cudaStream_t st) {
+    switch (p->nx) {
+        case 128:  return fwd ? launch_fused<128, true>(p, in, u, st) : launch_fused<128, false>(p, in, u, st);
+        case 256:  return fwd ? launch_fused<256, true>(p, in, u, st) : launch_fused<256, false>(p, in, u, st);
+        case 512:  return fwd ? launch_fused<512, true>(p, in, u, st) : launch_fused<512, false>(p, in, u, st);
+        case 1024: return fwd ? launch_fused<1024, true>(p, in, u, st) : launch_fused<1024, false>(p, in, u, st);
+        default:   return PP_ERR_UNSUPPORTED_SIZE;
+    }
+}
+
 int run_z(const pp_plan *p, double *w, cudaStream_t st) {
     ZParams zp;
     zp.nx = p->nx; zp.ny = p->ny; zp.nz = p->nz;
@@ -226,7 +277,7 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
 void free_plan(pp_plan *p) {
     if (!p) return;
     cudaFree(p->tw_x); cudaFree(p->tw_y); cudaFree(p->ptw_x); cudaFree(p->ptw_y);
-    cudaFree(p->sx); cudaFree(p->sy); cudaFree(p->zero_scratch); cudaFree(p->host_stage);
+    cudaFree(p->sx); cudaFree(p->sy); cudaFree(p->zero_scratch); cudaFree(p->host_stage); cudaFree(p->fuse_sync);
     for (auto &e : p->ev) if (e) cudaEventDestroy(e);
     cudaGetLastError();
     delete p;
@@ -274,6 +325,11 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
     p->dx = dx; p->dy = dy; p->dz = dz;
     p->bcx = bc_x; p->bcy = bc_y; p->bcz = bc_z;
     p->device = dev;
+    if (cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || p->num_sms <= 0) {
+        cudaGetLastError();
+        delete p;
+        return PP_ERR_CUDA;
+    }
     p->singular = (bc_x != PP_BC_DIRICHLET && bc_y != PP_BC_DIRICHLET && bc_z != PP_BC_DIRICHLET) ? 1 : 0;
     p->scale = (double)((long double)dz * (long double)dz / ((long double)nx * (long double)ny));
 
@@ -294,6 +350,11 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
     if (!rc) {
         std::vector<double> z((size_t)nz, 0.0);
         rc = upload(&p->zero_scratch, z, p->bytes);
+    }
+    if (!rc) {
+        const size_t nb = sizeof(int) * (size_t)(nz + 1);
+        if (cudaMalloc((void **)&p->fuse_sync, nb) != cudaSuccess) { p->fuse_sync = nullptr; cudaGetLastError(); rc = PP_ERR_ALLOC; }
+        else p->bytes += nb;
     }
     if (!rc) {
         for (auto &e : p->ev)
@@ -317,16 +378,27 @@ int pp_solve(const pp_plan *plan, const double *f, double *u, void *stream) {
     const bool prof = plan->profiling != 0;
     int rc;
 #define PP_MARK(i) if (prof && cudaEventRecord(mp->ev[i], st) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    const bool fused = plan->xy_fusion && fusion_supported(plan->nx, plan->ny);
     PP_MARK(0)
-    if ((rc = run_x(plan, true, f, u, st))) return rc;          // a1-a3: x pre / FFT / post
-    PP_MARK(1)
-    if ((rc = run_y(plan, true, u, st))) return rc;             // a4-a6: y pre / FFT / post
+    if (fused) {
+        if ((rc = run_fused(plan, true, f, u, st))) return rc;  // a1-a6 as tasks of one kernel
+        PP_MARK(1)
+    } else {
+        if ((rc = run_x(plan, true, f, u, st))) return rc;      // a1-a3: x pre / FFT / post
+        PP_MARK(1)
+        if ((rc = run_y(plan, true, u, st))) return rc;         // a4-a6: y pre / FFT / post
+    }
     PP_MARK(2)
     if ((rc = run_z(plan, u, st))) return rc;                   // a7-a8: diagonal + tridiagonal solve
     PP_MARK(3)
-    if ((rc = run_y(plan, false, u, st))) return rc;            // a9: y inverse
-    PP_MARK(4)
-    if ((rc = run_x(plan, false, u, u, st))) return rc;         // a10: x inverse
+    if (fused) {
+        PP_MARK(4)
+        if ((rc = run_fused(plan, false, u, u, st))) return rc; // a9-a10 as tasks of one kernel
+    } else {
+        if ((rc = run_y(plan, false, u, st))) return rc;        // a9: y inverse
+        PP_MARK(4)
+        if ((rc = run_x(plan, false, u, u, st))) return rc;     // a10: x inverse
+    }
     PP_MARK(5)
 #undef PP_MARK
     if (prof) mp->have_times = 1;
@@ -372,6 +444,13 @@ int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm) {
     if (algorithm == PP_Z_PARTITION && (plan->bcz == PP_BC_PERIODIC || zpart_shape(plan->nz).R == 0))
         return PP_ERR_UNSUPPORTED_SIZE;
     plan->z_algorithm = algorithm;
+    return PP_SUCCESS;
+}
+
+int pp_plan_set_xy_fusion(pp_plan *plan, int enable) {
+    if (!plan) return PP_ERR_NULL;
+    if (enable && !fusion_supported(plan->nx, plan->ny)) return PP_ERR_UNSUPPORTED_SIZE;
+    plan->xy_fusion = enable ? 1 : 0;
     return PP_SUCCESS;
 }
 

@@ -57,15 +57,16 @@ struct XCfg {
 // ------------------------------------------------------------------------------------------
 // forward: real rows -> spectral rows
 // ------------------------------------------------------------------------------------------
-template <int N>
-__global__ void __launch_bounds__(XCfg<N>::THREADS, PP_X_MINB)
-xpass_fwd_kernel(const double *in, double *out, long long npairs, int bc,
-                 const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
+// One CTA-wide tile of the forward x pass: T row pairs starting at pair0, P threads each
+// (blockDim.x == T * P).  `smem` holds T * FftCfg<N>::SMEM_ELEMS double2.
+template <int N, int T>
+__device__ __forceinline__ void xfwd_tile(const double *in, double *out, long long pair0, long long npairs, int bc,
+                                          const double2 *__restrict__ tw, const double2 *__restrict__ ptw,
+                                          double2 *smem) {
     using C = FftCfg<N>;
-    constexpr int E = C::E, P = C::P, T = XCfg<N>::T, H = N / 2;
-    extern __shared__ double2 smem[];
+    constexpr int E = C::E, P = C::P, H = N / 2;
     const int f = threadIdx.x / P, t = threadIdx.x % P;
-    const long long pair = (long long)blockIdx.x * T + f;
+    const long long pair = pair0 + f;
     const bool active = pair < npairs;
     const long long row = active ? pair * 2 : 0;
     const double *ra = in + row * N, *rb = ra + N;
@@ -144,18 +145,35 @@ xpass_fwd_kernel(const double *in, double *out, long long npairs, int bc,
     }
 }
 
+
+template <int N>
+__global__ void __launch_bounds__(XCfg<N>::THREADS, PP_X_MINB)
+xpass_fwd_kernel(const double *in, double *out, long long npairs, int bc,
+                 const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
+    extern __shared__ double2 smem[];
+    xfwd_tile<N, XCfg<N>::T>(in, out, (long long)blockIdx.x * XCfg<N>::T, npairs, bc, tw, ptw, smem);
+}
+
 // ------------------------------------------------------------------------------------------
 // inverse: spectral rows -> real rows
 // ------------------------------------------------------------------------------------------
-template <int N>
-__global__ void __launch_bounds__(XCfg<N>::THREADS, PP_X_MINB)
-xpass_inv_kernel(const double *in, double *out, long long npairs, int bc,
-                 const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
+// One CTA-wide tile of the inverse x pass (see xfwd_tile).  LDCG: read the input with ld.global.cg
+// (L2 only) -- for the fused y+x kernel, whose input rows were just written by other SMs.
+template <bool LDCG>
+__device__ __forceinline__ double xld(const double *p) { return LDCG ? __ldcg(p) : *p; }
+template <bool LDCG>
+__device__ __forceinline__ double2 xld2(const double *p) {
+    return LDCG ? __ldcg(reinterpret_cast<const double2 *>(p)) : *reinterpret_cast<const double2 *>(p);
+}
+
+template <int N, int T, bool LDCG>
+__device__ __forceinline__ void xinv_tile(const double *in, double *out, long long pair0, long long npairs, int bc,
+                                          const double2 *__restrict__ tw, const double2 *__restrict__ ptw,
+                                          double2 *smem) {
     using C = FftCfg<N>;
-    constexpr int E = C::E, P = C::P, T = XCfg<N>::T, H = N / 2;
-    extern __shared__ double2 smem[];
+    constexpr int E = C::E, P = C::P, H = N / 2;
     const int f = threadIdx.x / P, t = threadIdx.x % P;
-    const long long pair = (long long)blockIdx.x * T + f;
+    const long long pair = pair0 + f;
     const bool active = pair < npairs;
     const long long row = active ? pair * 2 : 0;
     const double *ra = in + row * N, *rb = ra + N;
@@ -171,8 +189,8 @@ xpass_inv_kernel(const double *in, double *out, long long npairs, int bc,
 #pragma unroll
         for (int q = 0; q < E / 2; ++q) {
             const int m = t + q * P;
-            const double2 A = *reinterpret_cast<const double2 *>(ra + 2 * m);
-            const double2 B = *reinterpret_cast<const double2 *>(rb + 2 * m);
+            const double2 A = xld2<LDCG>(ra + 2 * m);
+            const double2 B = xld2<LDCG>(rb + 2 * m);
             if (m == 0) {                                              // (X_0, X_{N/2}) of both rows, all real
                 v[q] = make_double2(A.x, B.x);
                 s[lay(H)] = make_double2(A.y, B.y);
@@ -193,14 +211,14 @@ xpass_inv_kernel(const double *in, double *out, long long npairs, int bc,
         } else {
             double ya, yb, yap, ybp;
             if (bc == BC_N) {
-                ya = ra[m]; yb = rb[m];
-                yap = (m == 0) ? 0.0 : ra[N - m];
-                ybp = (m == 0) ? 0.0 : rb[N - m];
+                ya = xld<LDCG>(ra + m); yb = xld<LDCG>(rb + m);
+                yap = (m == 0) ? 0.0 : xld<LDCG>(ra + N - m);
+                ybp = (m == 0) ? 0.0 : xld<LDCG>(rb + N - m);
             } else {                                                   // Y'_m = (-1)^m S_{N-1-m}
                 const double s1 = sgn_of(m);
-                ya = s1 * ra[N - 1 - m]; yb = s1 * rb[N - 1 - m];
-                yap = (m == 0) ? 0.0 : s1 * ra[m - 1];                 // (-1)^(N-m) S_{m-1}
-                ybp = (m == 0) ? 0.0 : s1 * rb[m - 1];
+                ya = s1 * xld<LDCG>(ra + N - 1 - m); yb = s1 * xld<LDCG>(rb + N - 1 - m);
+                yap = (m == 0) ? 0.0 : s1 * xld<LDCG>(ra + m - 1);                 // (-1)^(N-m) S_{m-1}
+                ybp = (m == 0) ? 0.0 : s1 * xld<LDCG>(rb + m - 1);
             }
             const double2 w = cconj(__ldg(&ptw[m]));
             v[q] = cmul(w, make_double2(ya + ybp, yb - yap));          // conj(w)^m (Y_m - i Y_{N-m})
@@ -228,6 +246,15 @@ xpass_inv_kernel(const double *in, double *out, long long npairs, int bc,
             }
         }
     }
+}
+
+
+template <int N>
+__global__ void __launch_bounds__(XCfg<N>::THREADS, PP_X_MINB)
+xpass_inv_kernel(const double *in, double *out, long long npairs, int bc,
+                 const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
+    extern __shared__ double2 smem[];
+    xinv_tile<N, XCfg<N>::T, false>(in, out, (long long)blockIdx.x * XCfg<N>::T, npairs, bc, tw, ptw, smem);
 }
 
 }  // namespace pp

@@ -52,17 +52,22 @@ struct YCfg {
 
 __device__ __forceinline__ double2 dscale(double a, double2 v) { return make_double2(a * v.x, a * v.y); }
 
-template <int N>
-__global__ void __launch_bounds__(YCfg<N>::THREADS, YCfg<N>::MINB)
-ypass_fwd_kernel(double2 *w, int nxh, int bc, int complex_cols,
-                 const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
+template <bool LDCG>
+__device__ __forceinline__ double2 yld(const double2 *p) { return LDCG ? __ldcg(p) : *p; }
+
+// One CTA-wide tile of the forward y pass: column tile bx (T double2 columns) of plane z, all N rows
+// (blockDim.x == T * FftCfg<N>::P).  `smem` holds T * FftCfg<N>::SMEM_ELEMS double2.  LDCG: read with
+// ld.global.cg -- for the fused x+y kernel, whose input was just written by other SMs.
+template <int N, bool LDCG>
+__device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int complex_cols,
+                                          const double2 *__restrict__ tw, const double2 *__restrict__ ptw,
+                                          int bx, int z, double2 *smem) {
     using C = FftCfg<N>;
     constexpr int E = C::E, P = C::P, T = YCfg<N>::T, H = N / 2;
-    extern __shared__ double2 smem[];
     const int c = threadIdx.x % T, t = threadIdx.x / T;
-    const int cp = blockIdx.x * T + c;
+    const int cp = bx * T + c;
     const bool active = cp < nxh;
-    double2 *base = w + (size_t)blockIdx.y * N * nxh + (active ? cp : 0);
+    double2 *base = w + (size_t)z * N * nxh + (active ? cp : 0);
     const size_t ld = nxh;
     const LayoutCol<T> lay{c};
     const SyncCta sync;
@@ -72,19 +77,19 @@ ypass_fwd_kernel(double2 *w, int nxh, int bc, int complex_cols,
     for (int q = 0; q < E; ++q) {
         const int i = t + q * P;
         if (bc == BC_P) {
-            v[q] = base[i * ld];
+            v[q] = yld<LDCG>(base + i * ld);
         } else if (bc == BC_N) {
             const int p = (i < H) ? 2 * i : 2 * (N - 1 - i) + 1;
-            v[q] = base[p * ld];
+            v[q] = yld<LDCG>(base + p * ld);
         } else {
-            if (i < H) v[q] = base[(N - 1 - 2 * i) * ld];
-            else       v[q] = dscale(-1.0, base[(2 * i - N) * ld]);
+            if (i < H) v[q] = yld<LDCG>(base + (N - 1 - 2 * i) * ld);
+            else       v[q] = dscale(-1.0, yld<LDCG>(base + (2 * i - N) * ld));
         }
     }
 
     fft<N, FWD>(v, t, smem, tw, lay, sync);
 
-    if (complex_cols && blockIdx.x > 0) {                  // block-uniform: all columns complex
+    if (complex_cols && bx > 0) {                  // block-uniform: all columns complex
         if (active) {
 #pragma unroll
             for (int q = 0; q < E; ++q) base[(t + q * P) * ld] = v[q];
@@ -142,17 +147,26 @@ ypass_fwd_kernel(double2 *w, int nxh, int bc, int complex_cols,
     }
 }
 
+
 template <int N>
 __global__ void __launch_bounds__(YCfg<N>::THREADS, YCfg<N>::MINB)
-ypass_inv_kernel(double2 *w, int nxh, int bc, int complex_cols,
+ypass_fwd_kernel(double2 *w, int nxh, int bc, int complex_cols,
                  const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
+    extern __shared__ double2 smem[];
+    yfwd_tile<N, false>(w, nxh, bc, complex_cols, tw, ptw, blockIdx.x, blockIdx.y, smem);
+}
+
+// One CTA-wide tile of the inverse y pass (see yfwd_tile).
+template <int N>
+__device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int complex_cols,
+                                          const double2 *__restrict__ tw, const double2 *__restrict__ ptw,
+                                          int bx, int z, double2 *smem) {
     using C = FftCfg<N>;
     constexpr int E = C::E, P = C::P, T = YCfg<N>::T, H = N / 2;
-    extern __shared__ double2 smem[];
     const int c = threadIdx.x % T, t = threadIdx.x / T;
-    const int cp = blockIdx.x * T + c;
+    const int cp = bx * T + c;
     const bool active = cp < nxh;
-    double2 *base = w + (size_t)blockIdx.y * N * nxh + (active ? cp : 0);
+    double2 *base = w + (size_t)z * N * nxh + (active ? cp : 0);
     const size_t ld = nxh;
     const LayoutCol<T> lay{c};
     const SyncCta sync;
@@ -205,6 +219,15 @@ ypass_inv_kernel(double2 *w, int nxh, int bc, int complex_cols,
             else            base[(N - 1 - p) * ld] = dscale(-sgn_of(p), v[q]);
         }
     }
+}
+
+
+template <int N>
+__global__ void __launch_bounds__(YCfg<N>::THREADS, YCfg<N>::MINB)
+ypass_inv_kernel(double2 *w, int nxh, int bc, int complex_cols,
+                 const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
+    extern __shared__ double2 smem[];
+    yinv_tile<N>(w, nxh, bc, complex_cols, tw, ptw, blockIdx.x, blockIdx.y, smem);
 }
 
 }  // namespace pp
