@@ -38,6 +38,7 @@ struct pp_plan {
     int z_algorithm;           // PP_Z_AUTO / PP_Z_SWEEP / PP_Z_PARTITION
     int xy_fusion;             // 1: x and y passes of a plane run as tasks of one kernel (pp_fused.cuh)
     int *fuse_sync;            // [1 + nz] ticket + per-plane completion counters
+    double *hier_scratch;      // [4][nz / 256][nx ny]: interface values of the two-level z solve (long lines only)
     cudaEvent_t ev[PP_NUM_KERNELS + 1];
 };
 
@@ -230,18 +231,34 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
 #ifndef PP_Z_CB
 #define PP_Z_CB 16
 #endif
-    const ZPartShape zs = (p->bcz != PP_BC_PERIODIC && p->z_algorithm != PP_Z_SWEEP) ? zpart_shape(p->nz) : ZPartShape{0, 0, 0};
+    const bool want_part = p->bcz != PP_BC_PERIODIC && p->z_algorithm != PP_Z_SWEEP;
+    const ZPartShape zs = want_part ? zpart_shape(p->nz) : ZPartShape{0, 0, 0};
     if (zs.R) {
         // partitioned, register-resident solve: one HBM read + one write per unknown (pp_zpart.cuh)
         const size_t ds = zpart_smem_bytes(zs);
         const unsigned grid = (unsigned)((plane + zs.L - 1) / zs.L);
+        const ZHier none = {1, nullptr, nullptr};
         if (zs.R == 32) {
-            if (int rc = set_smem(zsolve_part_kernel<32>, ds)) return rc;
-            zsolve_part_kernel<32><<<grid, zs.L * zs.S, ds, st>>>(w, zp, zs.S, zs.L);
+            if (int rc = set_smem(zsolve_part_kernel<32, 0>, ds)) return rc;
+            zsolve_part_kernel<32, 0><<<grid, zs.L * zs.S, ds, st>>>(w, zp, zs.S, zs.L, none);
         } else {
-            if (int rc = set_smem(zsolve_part_kernel<64>, ds)) return rc;
-            zsolve_part_kernel<64><<<grid, zs.L * zs.S, ds, st>>>(w, zp, zs.S, zs.L);
+            if (int rc = set_smem(zsolve_part_kernel<64, 0>, ds)) return rc;
+            zsolve_part_kernel<64, 0><<<grid, zs.L * zs.S, ds, st>>>(w, zp, zs.S, zs.L, none);
         }
+    } else if (want_part && p->hier_scratch) {
+        // long lines: two-level partition, 8 + 16 bytes per unknown (pp_zpart.cuh, ZHier)
+        const ZPartShape hs = {32, ZP_HIER_ROWS / 32, 32};
+        const size_t ds = zpart_smem_bytes(hs);
+        const int nK = p->nz / ZP_HIER_ROWS;
+        const size_t slab = (size_t)nK * plane;
+        const ZHier h = {nK, p->hier_scratch, p->hier_scratch + slab};
+        const dim3 grid((unsigned)((plane + hs.L - 1) / hs.L), (unsigned)nK);
+        if (int rc = set_smem(zsolve_part_kernel<32, 1>, ds)) return rc;
+        if (int rc = set_smem(zsolve_part_kernel<32, 2>, ds)) return rc;
+        zsolve_part_kernel<32, 1><<<grid, hs.L * hs.S, ds, st>>>(w, zp, hs.S, hs.L, h);
+        zsolve_hier_interface_kernel<<<(unsigned)((plane + 63) / 64), 64, 0, st>>>(zp, h, ZP_HIER_ROWS, p->hier_scratch + 2 * slab,
+                                                                             p->hier_scratch + 3 * slab);
+        zsolve_part_kernel<32, 2><<<grid, hs.L * hs.S, ds, st>>>(w, zp, hs.S, hs.L, h);
     } else if (p->bcz != PP_BC_PERIODIC) {
         // checkpoint table in shared memory: ceil(nz / CB) x TH doubles per CTA
 #define PP_ZT_LAUNCH(C, T)                                                                           \
@@ -277,7 +294,7 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
 void free_plan(pp_plan *p) {
     if (!p) return;
     cudaFree(p->tw_x); cudaFree(p->tw_y); cudaFree(p->ptw_x); cudaFree(p->ptw_y);
-    cudaFree(p->sx); cudaFree(p->sy); cudaFree(p->zero_scratch); cudaFree(p->host_stage); cudaFree(p->fuse_sync);
+    cudaFree(p->sx); cudaFree(p->sy); cudaFree(p->zero_scratch); cudaFree(p->host_stage); cudaFree(p->fuse_sync); cudaFree(p->hier_scratch);
     for (auto &e : p->ev) if (e) cudaEventDestroy(e);
     cudaGetLastError();
     delete p;
@@ -313,7 +330,10 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
         return PP_ERR_INVALID_ARG;
     for (int bc : {bc_x, bc_y, bc_z})
         if (bc != PP_BC_PERIODIC && bc != PP_BC_NEUMANN && bc != PP_BC_DIRICHLET) return PP_ERR_INVALID_ARG;
-    if (!pow2_in_range(nx) || !pow2_in_range(ny) || nz < 2 || nz > 64 * Z_MAX_CK) return PP_ERR_UNSUPPORTED_SIZE;
+    // nz: the two-sweep kernels take any nz up to 4096; longer lines need the two-level partition
+    // (Neumann / Dirichlet z, nz a multiple of 256 up to 32768)
+    const bool long_ok = bc_z != PP_BC_PERIODIC && zpart_hier_ok(nz);
+    if (!pow2_in_range(nx) || !pow2_in_range(ny) || nz < 2 || (nz > 64 * Z_MAX_CK && !long_ok)) return PP_ERR_UNSUPPORTED_SIZE;
 
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
@@ -350,6 +370,11 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
     if (!rc) {
         std::vector<double> z((size_t)nz, 0.0);
         rc = upload(&p->zero_scratch, z, p->bytes);
+    }
+    if (!rc && long_ok && zpart_shape(nz).R == 0) {
+        const size_t nb = sizeof(double) * 4 * (size_t)(nz / ZP_HIER_ROWS) * (size_t)nx * (size_t)ny;
+        if (cudaMalloc((void **)&p->hier_scratch, nb) != cudaSuccess) { p->hier_scratch = nullptr; cudaGetLastError(); rc = PP_ERR_ALLOC; }
+        else p->bytes += nb;
     }
     if (!rc) {
         const size_t nb = sizeof(int) * (size_t)(nz + 1);
@@ -441,8 +466,9 @@ int pp_plan_set_profiling(pp_plan *plan, int enable) {
 int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm) {
     if (!plan) return PP_ERR_NULL;
     if (algorithm != PP_Z_AUTO && algorithm != PP_Z_SWEEP && algorithm != PP_Z_PARTITION) return PP_ERR_INVALID_ARG;
-    if (algorithm == PP_Z_PARTITION && (plan->bcz == PP_BC_PERIODIC || zpart_shape(plan->nz).R == 0))
+    if (algorithm == PP_Z_PARTITION && (plan->bcz == PP_BC_PERIODIC || (zpart_shape(plan->nz).R == 0 && !plan->hier_scratch)))
         return PP_ERR_UNSUPPORTED_SIZE;
+    if (algorithm == PP_Z_SWEEP && plan->nz > 64 * Z_MAX_CK) return PP_ERR_UNSUPPORTED_SIZE;
     plan->z_algorithm = algorithm;
     return PP_SUCCESS;
 }

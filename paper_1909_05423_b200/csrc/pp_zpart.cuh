@@ -56,6 +56,10 @@ inline ZPartShape zpart_shape(int nz) {
     return {0, 0, 0};
 }
 
+// long lines: super-segments of 256 rows (R = 32, S = 8), nz a multiple of 256, at least two of them
+constexpr int ZP_HIER_ROWS = 256;
+inline bool zpart_hier_ok(int nz) { return nz % ZP_HIER_ROWS == 0 && nz / ZP_HIER_ROWS >= 2 && nz <= 32768; }
+
 // dynamic shared memory of one CTA, in doubles:
 //   Q [2][R+1][L]   leading minors of the first (0) and interior (1) block
 //   G [2][R][L]     pivots g_i
@@ -90,9 +94,24 @@ __device__ __forceinline__ void zp_minors(double d0, double dint, double dlast, 
     qR = qc;
 }
 
-template <int R>
+// Long systems (nz beyond what one CTA holds): the same partition one level up.  The line is cut into
+// nK super-segments of R S rows, one CTA each (blockIdx.y), every one an R S x R S block of the same
+// Toeplitz matrix:
+//   MODE 1  solves each super-segment as if isolated (neighbours = 0) and writes only its first and
+//           last unknown to HF[K], HL[K]                                  (reads 8 B/point)
+//   zsolve_hier_interface_kernel couples the super-segments: the same 2x2-block interface system,
+//           one thread per mode, leaving x just above / below every super-segment in HL[K-1], HF[K+1]
+//   MODE 2  solves each super-segment again with those neighbour values moved to the right-hand
+//           side and stores the solution                                   (8 B read + 8 B write)
+// MODE 0 is the whole line in one CTA (nK = 1).
+struct ZHier {
+    int nK;                  // super-segments per line
+    double *HF, *HL;         // [nK][plane]
+};
+
+template <int R, int MODE>
 __global__ void __launch_bounds__(PP_ZP_MAXT, (R == 32) ? PP_ZP_MINB : PP_ZP_MINB / 2)
-zsolve_part_kernel(double *w, ZParams p, int S, int L) {
+zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
     static_assert(R % 2 == 0, "the spike signs below assume an even segment length");
     extern __shared__ double zsm[];
     double *Q = zsm;                                  // [2][R+1][L]
@@ -109,17 +128,25 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L) {
     const size_t e = (size_t)blockIdx.x * L + l;
     const bool live = e < plane;
     const bool pin = !live || (p.singular && e == 0);       // pinned line: computed with a placeholder, never stored
-    const bool mirror = (S > 1) && (j == S - 1);              // last segment: rows held in reverse order
-    const int c = (j == 0 || j == S - 1) ? 0 : 1;             // which block: first (and mirrored last) / interior
+    const int K = (MODE == 0) ? 0 : (int)blockIdx.y;         // super-segment of this CTA
+    const bool top_end = (MODE == 0) || K == 0;               // the CTA's rows start at the line's first row
+    const bool bot_end = (MODE == 0) || K == h.nK - 1;        // ... end at its last row
+    const bool mirror = bot_end && (S > 1) && (j == S - 1);   // line's last segment: rows held in reverse order
+    const int c = ((j == 0 && top_end) || (j == S - 1 && bot_end)) ? 0 : 1;   // first (and mirrored last) / interior block
     // row i of the segment lives at row0 + i * step (the mirrored segment walks upwards)
     const ptrdiff_t step = mirror ? -(ptrdiff_t)plane : (ptrdiff_t)plane;
-    double *row0 = w + (live ? e : 0) + ((size_t)j * R + (mirror ? R - 1 : 0)) * plane;
+    double *row0 = w + (live ? e : 0) + (((size_t)K * S + j) * R + (mirror ? R - 1 : 0)) * plane;
 
     // the mode's shift first (the tabulating threads start from it), then every right-hand side of
     // the segment, in flight at once
     const int jfac = (S >= 3) ? 2 : 1;
     double s = -1.0;
     if (j <= jfac && !pin) s = __ldg(p.sx + (int)(e % p.nx)) + __ldg(p.sy + (int)(e / p.nx));
+    double ext0 = 0.0, ext1 = 0.0;                            // x just above the CTA's first row / below its last
+    if (MODE == 2 && live) {
+        if (j == 0 && !top_end) ext0 = h.HL[(size_t)(K - 1) * plane + e];
+        if (j == S - 1 && !bot_end) ext1 = h.HF[(size_t)(K + 1) * plane + e];
+    }
     double y[R];
 #pragma unroll
     for (int i = 0; i < R; ++i) y[i] = __ldcs(row0 + i * step);
@@ -155,16 +182,17 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L) {
                 im = ic; ic = in;
             }
             const double rqe = fast_rcp(ec), rqi = fast_rcp(ic);
+            const double a1 = (S >= 3 || MODE != 0) ? im * rqi : 0.0, b1 = (S >= 3 || MODE != 0) ? -rqi : 0.0;
             const double a0 = em * rqe;
-            const double a1 = (S >= 3) ? im * rqi : 0.0, b1 = (S >= 3) ? -rqi : 0.0;
+            const double atop = top_end ? a0 : a1, abot = bot_end ? a0 : a1;
             // A_J obeys the Moebius recurrence A_0 = a0, A_J = a1 + b1^2 A_{J-1} / (1 - a1 A_{J-1}); carried
             // as the ratio N_J / M_J it is two FMAs per step, and the reciprocals leave the dependency chain:
             //   D_J = M_J / (M_J - vF_J N_J),   (A D)_J = N_J / (M_J - vF_J N_J)
             const double k1 = fma(b1, b1, -a1 * a1);
-            double N = a0, M = 1.0;
+            double N = atop, M = 1.0;
             for (int J = 0; J < S - 1; ++J) {
                 const double vL = (J == 0) ? 0.0 : b1;
-                const double vF = (J + 1 == S - 1) ? a0 : a1, wF = (J + 1 == S - 1) ? 0.0 : b1;
+                const double vF = (J + 1 == S - 1) ? abot : a1, wF = (J + 1 == S - 1) ? 0.0 : b1;
                 const double r = fast_rcp(fma(-vF, N, M));
                 const double D = M * r, AD = N * r;
                 double *f = F + J * L + l;
@@ -186,8 +214,8 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L) {
         const double *gt = G + c * R * L + l;
         const double *gb = G + ((S == 1) ? 0 : R * L) + l;
         const double scale = p.scale;
-        y[0] = y[0] * scale * gt[0];
-        y[R - 1] = y[R - 1] * scale * gb[0];
+        y[0] = fma(y[0], scale, -ext0) * gt[0];
+        y[R - 1] = fma(y[R - 1], scale, -ext1) * gb[0];
 #pragma unroll
         for (int k = 1; k < M; ++k) {
             y[k] = fma(y[k], scale, -y[k - 1]) * gt[k * L];
@@ -260,6 +288,12 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L) {
             if (i % 8 == 6) zp_sched_fence();
         }
     }
+    if (MODE == 1) {
+        // first and last unknown of the isolated super-segment (an end of the line needs only one of them)
+        if (live && j == 0) h.HF[(size_t)K * plane + e] = y[0];
+        if (live && j == S - 1) h.HL[(size_t)K * plane + e] = mirror ? y[0] : y[R - 1];
+        return;
+    }
     if (!pin) {
         // recompute the row addresses instead of keeping the R load addresses alive (registers)
         double *out0 = row0;
@@ -269,7 +303,61 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L) {
         for (int i = 0; i < R; ++i) __stcs(out0 + i * ostep, y[i]);
     }
     // the warp that owns element 0 solves the singular line together (its line was never stored above)
-    if (p.singular && blockIdx.x == 0 && threadIdx.x < 32) zero_mode_line(w, plane, p.nz, p.bcz, p.scale, p.zero_scratch);
+    if (p.singular && blockIdx.x == 0 && K == 0 && threadIdx.x < 32) zero_mode_line(w, plane, p.nz, p.bcz, p.scale, p.zero_scratch);
+}
+
+// Couples the super-segments of every line (see ZHier): one thread per mode.  The super-segment block
+// is the rows x rows Toeplitz block; its couplings are ratios and products of its Thomas pivots
+// g_k = 1 / (d_k - g_{k-1}) (no minors here: q_rows would overflow for rows = 256):
+//   a1 = g_{rows-1} (interior block),  a0 = g_{rows-1} (end block, d_0 = b_end),  b1 = -prod_k g_k.
+// Same interface system and the same Moebius form of its factorisation as inside the CTA.
+// In: HF[K], HL[K] = first / last unknown of the isolated super-segment K.
+// Out: HL[K] = x of the last row of super-segment K (K < nK-1), HF[K] = x of the first row of
+// super-segment K (K > 0).  SC, SA: [nK][plane] scratch.
+__global__ void __launch_bounds__(64)
+zsolve_hier_interface_kernel(ZParams p, ZHier h, int rows, double *SC, double *SA) {
+    const size_t plane = (size_t)p.nx * p.ny;
+    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= plane || (p.singular && e == 0)) return;
+    const double s = p.sx[e % p.nx] + p.sy[e / p.nx];
+    const double bint = -2.0 + s;
+    const double bend = ((p.bcz == 1) ? -1.0 : -3.0) + s;
+    double gi = fast_rcp(bint), ge = fast_rcp(bend), prod = gi;
+    for (int k = 1; k < rows; ++k) {
+        gi = fast_rcp(bint - gi);
+        ge = fast_rcp(bint - ge);
+        prod *= gi;
+    }
+    const double a0 = ge, a1 = gi, b1 = -prod;
+    const int nK = h.nK;
+    const double k1 = fma(b1, b1, -a1 * a1);
+    double N = a0, M = 1.0, pa = 0.0;
+    for (int J = 0; J < nK - 1; ++J) {
+        const double vL = (J == 0) ? 0.0 : b1;
+        const double vF = (J + 1 == nK - 1) ? a0 : a1, wF = (J + 1 == nK - 1) ? 0.0 : b1;
+        const double r = fast_rcp(fma(-vF, N, M));
+        const double D = M * r, AD = N * r;
+        const double Ya = fma(-vL, pa, h.HL[(size_t)J * plane + e]);
+        const double t = fma(-vF, Ya, h.HF[(size_t)(J + 1) * plane + e]);
+        pa = fma(-AD, t, Ya);
+        h.HF[(size_t)(J + 1) * plane + e] = D * t;          // pc_J
+        h.HL[(size_t)J * plane + e] = pa;                   // pa_J
+        SC[(size_t)J * plane + e] = D * wF;
+        SA[(size_t)J * plane + e] = -AD * wF;
+        const double Nn = fma(k1, N, a1 * M), Mn = fma(-a1, N, M);
+        // keep the pair (N, M) near 1: only its ratio matters
+        const double nrm = fast_rcp(fabs(Mn) > fabs(Nn) ? Mn : Nn);
+        N = Nn * nrm;
+        M = Mn * nrm;
+    }
+    double cn = 0.0;
+    for (int J = nK - 2; J >= 0; --J) {
+        const double cv = fma(-SC[(size_t)J * plane + e], cn, h.HF[(size_t)(J + 1) * plane + e]);
+        const double av = fma(-SA[(size_t)J * plane + e], cn, h.HL[(size_t)J * plane + e]);
+        h.HF[(size_t)(J + 1) * plane + e] = cv;             // first row of super-segment J+1
+        h.HL[(size_t)J * plane + e] = av;                   // last row of super-segment J
+        cn = cv;
+    }
 }
 
 }  // namespace pp

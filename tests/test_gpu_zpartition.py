@@ -65,3 +65,46 @@ def test_partition_refused_where_it_does_not_apply():
         plan.set_z_algorithm("sweep")
         plan.set_z_algorithm("auto")
         plan.destroy()
+
+
+# ---------------------------------------------------------------- long lines: two-level partition
+@pytest.mark.parametrize("nz", [512 + 256, 1280, 2304, 4096])
+@pytest.mark.parametrize("combo", ["PPN", "NND", "DDD", "NNN"])
+def test_two_level_partition_matches_oracle(nz, combo):
+    """nz = 256 m that no single CTA holds: super-segments of 256 rows coupled by the interface
+    kernel.  At nz <= 4096 the two-sweep kernel solves the same systems: both must match the oracle."""
+    bc = wl.parse_bc(combo)
+    shape = (nz, 4, 24 if False else 16)
+    h = (1.0 / 16, 1.0 / 4, 1.0 / 8)
+    f = wl.random_normal(shape, 2000 + nz, zero_mean=all(b in (0, 1) for b in bc))
+    ref = po.solve(f, h, bc)
+    for alg in ("partition", "sweep"):
+        e = rel_err(gpu_solve(f, h, bc, z_algorithm=alg), ref)
+        assert e <= TOL, (alg, nz, combo, e)
+
+
+@pytest.mark.parametrize("combo", ["PPD", "PPN"])
+def test_paper_pencil_shape(combo):
+    """64 x 64 x 16384, the paper's per-GPU weak-scaling load: beyond the two-sweep
+    kernel's range, solved by the two-level partition only."""
+    w = wl.paper_pencil(combo)
+    # Lines this long are ill-conditioned (cond(T) ~ nz^2 for the lowest modes): an fp64 Thomas sweep
+    # is itself only good to ~1e-11 here, so the ground truth is the oracle with its z solve in
+    # long double (oracle/poisson_oracle.py, zdtype; SURVEY.md 8(c) "precision hazards").
+    ref = po.solve(w.f, w.h, w.bc, zdtype=np.longdouble)
+    u = gpu_solve(w.f, w.h, w.bc)
+    e = rel_err(u, ref)
+    assert e <= TOL, (combo, e)
+    e64 = rel_err(po.solve(w.f, w.h, w.bc), ref)
+    print(f"pencil {combo}: gpu vs long-double oracle {e:.2e}; fp64 oracle vs long-double oracle {e64:.2e}")
+
+
+def test_long_line_limits():
+    import paper_1909_05423_b200 as pp
+    for nz, combo, ok in ((8192, "PPN", True), (8192, "PPP", False), (8192 + 128, "PPN", False), (65536, "PPD", False)):
+        st, h = pp.binding.pp_plan_create(8, 8, nz, 0.1, 0.1, 0.1, *wl.parse_bc(combo))
+        assert (st == 0) == ok, (nz, combo, st)
+        if h:
+            if ok:
+                assert pp.binding.pp_plan_set_z_algorithm(h, pp.binding.PP_Z_SWEEP) != 0
+            pp.binding.pp_plan_destroy(h)
