@@ -51,7 +51,7 @@ enum { PP_BC_PERIODIC = 0, PP_BC_NEUMANN = 1, PP_BC_DIRICHLET = 2 };
 enum {
     PP_SUCCESS = 0,
     PP_ERR_INVALID_ARG = 1,      /* non-positive size/spacing, unknown BC, misaligned or partially overlapping pointers */
-    PP_ERR_UNSUPPORTED_SIZE = 2, /* nx or ny not a power of two in [4, 2048]; nz outside [2, 4096] */
+    PP_ERR_UNSUPPORTED_SIZE = 2, /* nx or ny not a power of two in [4, 2048]; nz outside [2, 4096] (long lines: see pp_plan_create) */
     PP_ERR_ALLOC = 3,            /* host or device allocation failed */
     PP_ERR_CUDA = 4,             /* a CUDA runtime call or kernel launch failed (no device, bad stream, ...) */
     PP_ERR_NULL = 5              /* a required pointer argument is NULL */
@@ -65,7 +65,9 @@ enum { PP_K_XFWD = 0, PP_K_YFWD = 1, PP_K_ZSOLVE = 2, PP_K_YINV = 3, PP_K_XINV =
  * bc_x, bc_y, bc_z (PP_BC_*).  Mirrors the paper's construction "PoissonGPU(n0,n1,n2)" +
  * "assignBoundary(bc)" (Listing 3).
  *   out      : host pointer receiving the handle (set to NULL on failure).
- *   nx, ny   : powers of two in [4, 2048] (the hand-written FFT core);  nz in [2, 4096].
+ *   nx, ny   : powers of two in [4, 2048] (the hand-written FFT core);  nz in [2, 4096], or -- with
+ *              Neumann / Dirichlet z -- any multiple of 256 up to 16384 (the paper's 64 x 64 x 16384
+ *              pencils; solved by the two-level partition, see pp_plan_set_z_algorithm).
  * Synchronous.  Builds the twiddle, post-twiddle and modified-wavenumber tables on the host
  * in extended precision and uploads them to the CURRENT device; the plan is bound to it.
  */
@@ -117,8 +119,11 @@ int pp_plan_last_kernel_ms(pp_plan *plan, float *ms_out);
  *   PP_Z_PARTITION : each system cut into segments of 32 or 64 rows held in registers and
  *                    coupled through their interface unknowns (the reduction idea of CR-P,
  *                    PAPER.md:250-258, across the threads of one CTA).  Needs Neumann or
- *                    Dirichlet z and nz = 32 m or 64 m (m <= 8), 1024 or 2048; otherwise
- *                    PP_ERR_UNSUPPORTED_SIZE and the plan is left unchanged.
+ *                    Dirichlet z and nz = 32 m or 64 m (m <= 8), 1024 or 2048 -- or nz = 256 m
+ *                    (2 <= m <= 64), where the same partition is applied on two levels
+ *                    (super-segments of 256 rows, three kernels); otherwise
+ *                    PP_ERR_UNSUPPORTED_SIZE and the plan is left unchanged.  PP_Z_SWEEP is
+ *                    refused for nz > 4096.
  */
 enum { PP_Z_AUTO = 0, PP_Z_SWEEP = 1, PP_Z_PARTITION = 2 };
 int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm);

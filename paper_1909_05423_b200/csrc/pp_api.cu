@@ -259,6 +259,7 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
         zsolve_hier_interface_kernel<<<(unsigned)((plane + 63) / 64), 64, 0, st>>>(zp, h, ZP_HIER_ROWS, p->hier_scratch + 2 * slab,
                                                                              p->hier_scratch + 3 * slab);
         zsolve_part_kernel<32, 2><<<grid, hs.L * hs.S, ds, st>>>(w, zp, hs.S, hs.L, h);
+        if (p->singular) zero_mode_long_kernel<<<1, 1024, 0, st>>>(w, plane, p->nz, p->scale);
     } else if (p->bcz != PP_BC_PERIODIC) {
         // checkpoint table in shared memory: ceil(nz / CB) x TH doubles per CTA
 #define PP_ZT_LAUNCH(C, T)                                                                           \
@@ -313,7 +314,7 @@ const char *pp_strerror(int status) {
     switch (status) {
         case PP_SUCCESS: return "success";
         case PP_ERR_INVALID_ARG: return "invalid argument";
-        case PP_ERR_UNSUPPORTED_SIZE: return "unsupported grid size (nx, ny: powers of two in [4, 2048]; nz in [2, 4096])";
+        case PP_ERR_UNSUPPORTED_SIZE: return "unsupported grid size (nx, ny: powers of two in [4, 2048]; nz in [2, 4096], or 256 m <= 16384 with non-periodic z)";
         case PP_ERR_ALLOC: return "allocation failed";
         case PP_ERR_CUDA: return "CUDA runtime or launch error (is a CUDA device present?)";
         case PP_ERR_NULL: return "null pointer argument";
@@ -331,7 +332,7 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
     for (int bc : {bc_x, bc_y, bc_z})
         if (bc != PP_BC_PERIODIC && bc != PP_BC_NEUMANN && bc != PP_BC_DIRICHLET) return PP_ERR_INVALID_ARG;
     // nz: the two-sweep kernels take any nz up to 4096; longer lines need the two-level partition
-    // (Neumann / Dirichlet z, nz a multiple of 256 up to 32768)
+    // (Neumann / Dirichlet z, nz a multiple of 256 up to 16384)
     const bool long_ok = bc_z != PP_BC_PERIODIC && zpart_hier_ok(nz);
     if (!pow2_in_range(nx) || !pow2_in_range(ny) || nz < 2 || (nz > 64 * Z_MAX_CK && !long_ok)) return PP_ERR_UNSUPPORTED_SIZE;
 

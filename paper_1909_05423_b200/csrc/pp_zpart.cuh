@@ -58,7 +58,7 @@ inline ZPartShape zpart_shape(int nz) {
 
 // long lines: super-segments of 256 rows (R = 32, S = 8), nz a multiple of 256, at least two of them
 constexpr int ZP_HIER_ROWS = 256;
-inline bool zpart_hier_ok(int nz) { return nz % ZP_HIER_ROWS == 0 && nz / ZP_HIER_ROWS >= 2 && nz <= 32768; }
+inline bool zpart_hier_ok(int nz) { return nz % ZP_HIER_ROWS == 0 && nz / ZP_HIER_ROWS >= 2 && nz <= 16384; }
 
 // dynamic shared memory of one CTA, in doubles:
 //   Q [2][R+1][L]   leading minors of the first (0) and interior (1) block
@@ -303,7 +303,8 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
         for (int i = 0; i < R; ++i) __stcs(out0 + i * ostep, y[i]);
     }
     // the warp that owns element 0 solves the singular line together (its line was never stored above)
-    if (p.singular && blockIdx.x == 0 && K == 0 && threadIdx.x < 32) zero_mode_line(w, plane, p.nz, p.bcz, p.scale, p.zero_scratch);
+    // (long lines: zero_mode_long_kernel does it with a whole CTA)
+    if (MODE == 0 && p.singular && blockIdx.x == 0 && threadIdx.x < 32) zero_mode_line(w, plane, p.nz, p.bcz, p.scale, p.zero_scratch);
 }
 
 // Couples the super-segments of every line (see ZHier): one thread per mode.  The super-segment block
@@ -322,42 +323,150 @@ zsolve_hier_interface_kernel(ZParams p, ZHier h, int rows, double *SC, double *S
     const double s = p.sx[e % p.nx] + p.sy[e / p.nx];
     const double bint = -2.0 + s;
     const double bend = ((p.bcz == 1) ? -1.0 : -3.0) + s;
-    double gi = fast_rcp(bint), ge = fast_rcp(bend), prod = gi;
-    for (int k = 1; k < rows; ++k) {
-        gi = fast_rcp(bint - gi);
-        ge = fast_rcp(bint - ge);
-        prod *= gi;
+    // pivots of the super-segment block from its leading minors (one FMA per row), renormalised every
+    // 32 rows so that nothing overflows:  g_{rows-1} = q_{rows-1} / q_rows,  prod_k g_k = 1 / q_rows
+    double im = 1.0, ic = bint, em = 1.0, ec = bend, prod = 1.0;
+    for (int k0 = 1; k0 < rows; k0 += 32) {
+#pragma unroll
+        for (int k = 0; k < 32; ++k) {
+            if (k0 + k < rows) {
+                const double in = fma(bint, ic, -im), en = fma(bint, ec, -em);
+                im = ic; ic = in;
+                em = ec; ec = en;
+            }
+        }
+        const double ri = fast_rcp(ic), re = fast_rcp(ec);
+        prod *= ri;                       // underflows to 0 for strongly dominant modes: the coupling is 0 then
+        im *= ri; ic = 1.0;
+        em *= re; ec = 1.0;
     }
-    const double a0 = ge, a1 = gi, b1 = -prod;
+    const double a0 = em, a1 = im, b1 = -prod;
     const int nK = h.nK;
     const double k1 = fma(b1, b1, -a1 * a1);
     double N = a0, M = 1.0, pa = 0.0;
-    for (int J = 0; J < nK - 1; ++J) {
-        const double vL = (J == 0) ? 0.0 : b1;
-        const double vF = (J + 1 == nK - 1) ? a0 : a1, wF = (J + 1 == nK - 1) ? 0.0 : b1;
-        const double r = fast_rcp(fma(-vF, N, M));
-        const double D = M * r, AD = N * r;
-        const double Ya = fma(-vL, pa, h.HL[(size_t)J * plane + e]);
-        const double t = fma(-vF, Ya, h.HF[(size_t)(J + 1) * plane + e]);
-        pa = fma(-AD, t, Ya);
-        h.HF[(size_t)(J + 1) * plane + e] = D * t;          // pc_J
-        h.HL[(size_t)J * plane + e] = pa;                   // pa_J
-        SC[(size_t)J * plane + e] = D * wF;
-        SA[(size_t)J * plane + e] = -AD * wF;
-        const double Nn = fma(k1, N, a1 * M), Mn = fma(-a1, N, M);
-        // keep the pair (N, M) near 1: only its ratio matters
-        const double nrm = fast_rcp(fabs(Mn) > fabs(Nn) ? Mn : Nn);
-        N = Nn * nrm;
-        M = Mn * nrm;
+    constexpr int CH = 8;                 // interface values are fetched CH steps at a time (the loop is latency bound)
+    for (int J0 = 0; J0 < nK - 1; J0 += CH) {
+        double yl[CH], yf[CH];
+#pragma unroll
+        for (int i = 0; i < CH; ++i) {
+            const int J = min(J0 + i, nK - 2);
+            yl[i] = h.HL[(size_t)J * plane + e];
+            yf[i] = h.HF[(size_t)(J + 1) * plane + e];
+        }
+#pragma unroll
+        for (int i = 0; i < CH; ++i) {
+            const int J = J0 + i;
+            if (J < nK - 1) {
+                const double vL = (J == 0) ? 0.0 : b1;
+                const double vF = (J + 1 == nK - 1) ? a0 : a1, wF = (J + 1 == nK - 1) ? 0.0 : b1;
+                const double r = fast_rcp(fma(-vF, N, M));
+                const double D = M * r, AD = N * r;
+                const double Ya = fma(-vL, pa, yl[i]);
+                const double t = fma(-vF, Ya, yf[i]);
+                pa = fma(-AD, t, Ya);
+                h.HF[(size_t)(J + 1) * plane + e] = D * t;          // pc_J
+                h.HL[(size_t)J * plane + e] = pa;                   // pa_J
+                SC[(size_t)J * plane + e] = D * wF;
+                SA[(size_t)J * plane + e] = -AD * wF;
+                const double Nn = fma(k1, N, a1 * M), Mn = fma(-a1, N, M);
+                // keep the pair (N, M) near 1: only its ratio matters
+                const double nrm = fast_rcp(fabs(Mn) > fabs(Nn) ? Mn : Nn);
+                N = Nn * nrm;
+                M = Mn * nrm;
+            }
+        }
     }
     double cn = 0.0;
-    for (int J = nK - 2; J >= 0; --J) {
-        const double cv = fma(-SC[(size_t)J * plane + e], cn, h.HF[(size_t)(J + 1) * plane + e]);
-        const double av = fma(-SA[(size_t)J * plane + e], cn, h.HL[(size_t)J * plane + e]);
-        h.HF[(size_t)(J + 1) * plane + e] = cv;             // first row of super-segment J+1
-        h.HL[(size_t)J * plane + e] = av;                   // last row of super-segment J
-        cn = cv;
+    for (int J0 = nK - 2; J0 >= 0; J0 -= CH) {
+        double sc[CH], sa[CH], pc[CH], pv[CH];
+#pragma unroll
+        for (int i = 0; i < CH; ++i) {
+            const int J = max(J0 - i, 0);
+            sc[i] = SC[(size_t)J * plane + e];
+            sa[i] = SA[(size_t)J * plane + e];
+            pc[i] = h.HF[(size_t)(J + 1) * plane + e];
+            pv[i] = h.HL[(size_t)J * plane + e];
+        }
+#pragma unroll
+        for (int i = 0; i < CH; ++i) {
+            const int J = J0 - i;
+            if (J >= 0) {
+                const double cv = fma(-sc[i], cn, pc[i]);
+                const double av = fma(-sa[i], cn, pv[i]);
+                h.HF[(size_t)(J + 1) * plane + e] = cv;             // first row of super-segment J+1
+                h.HL[(size_t)J * plane + e] = av;                   // last row of super-segment J
+                cn = cv;
+            }
+        }
     }
+}
+
+// The singular (0,0) line of a long Neumann-z problem (R11), by one CTA of
+// 1024 threads: the same two running sums as zero_mode_line, each thread holding its contiguous
+// chunk of at most 16 rows in registers (nz <= 16384), chunk totals combined by block-wide scans.
+//   r <- (r - mean r) scale;  x_0 = 0;  d_k = -sum_{m >= k} r_m;  x_k = sum_{1 <= m <= k} d_m;  x <- x - mean x
+__device__ __forceinline__ double zp_block_excl_scan(double v, double *red, double &total) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const double wex = warp_excl_scan(v, lane);
+    const double wtot = __shfl_sync(0xffffffffu, wex + v, 31);
+    __syncthreads();                                          // red may still be read from the previous call
+    if (lane == 0) red[wid] = wtot;
+    __syncthreads();
+    const double mine = (lane < nw) ? red[lane] : 0.0;
+    const double wprefix = warp_excl_scan(mine, lane);
+    total = __shfl_sync(0xffffffffu, wprefix + mine, 31);
+    return __shfl_sync(0xffffffffu, wprefix, wid) + wex;
+}
+
+__global__ void __launch_bounds__(1024, 1)
+zero_mode_long_kernel(double *col, size_t plane, int nz, double scale) {
+    __shared__ double red[32];
+    constexpr int C = 16;
+    const int c = (nz + (int)blockDim.x - 1) / (int)blockDim.x;        // <= C
+    const int k0 = min((int)threadIdx.x * c, nz), k1 = min(k0 + c, nz);
+    double v[C];
+    double acc = 0.0, tot;
+#pragma unroll
+    for (int i = 0; i < C; ++i) {
+        v[i] = (i < c && k0 + i < k1) ? col[(size_t)(k0 + i) * plane] * scale : 0.0;
+        acc += v[i];
+    }
+    zp_block_excl_scan(acc, red, tot);
+    const double mean = tot / nz;
+    // rows >= 1 only; v <- r - mean
+    double own = 0.0;
+#pragma unroll
+    for (int i = 0; i < C; ++i) {
+        const bool in = i < c && k0 + i < k1 && k0 + i >= 1;
+        v[i] = in ? v[i] - mean : 0.0;
+        own += v[i];
+    }
+    double all;
+    double run = zp_block_excl_scan(own, red, all);
+    double dsum = 0.0;
+#pragma unroll
+    for (int i = 0; i < C; ++i) {
+        const bool in = i < c && k0 + i < k1 && k0 + i >= 1;
+        const double r = v[i];
+        v[i] = in ? -(all - run) : 0.0;                               // d_k
+        run += r;
+        dsum += v[i];
+    }
+    double dummy;
+    double x = zp_block_excl_scan(dsum, red, dummy);
+    double xs = 0.0;
+#pragma unroll
+    for (int i = 0; i < C; ++i) {
+        x += v[i];
+        v[i] = x;                                                     // x_k (x_0 = 0)
+        if (i < c && k0 + i < k1) xs += x;
+    }
+    double xtot;
+    zp_block_excl_scan(xs, red, xtot);
+    const double xmean = xtot / nz;
+#pragma unroll
+    for (int i = 0; i < C; ++i)
+        if (i < c && k0 + i < k1) col[(size_t)(k0 + i) * plane] = v[i] - xmean;
 }
 
 }  // namespace pp

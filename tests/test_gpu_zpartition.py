@@ -101,7 +101,7 @@ def test_paper_pencil_shape(combo):
 
 def test_long_line_limits():
     import paper_1909_05423_b200 as pp
-    for nz, combo, ok in ((8192, "PPN", True), (8192, "PPP", False), (8192 + 128, "PPN", False), (65536, "PPD", False)):
+    for nz, combo, ok in ((8192, "PPN", True), (8192, "PPP", False), (8192 + 128, "PPN", False), (32768, "PPD", False)):
         st, h = pp.binding.pp_plan_create(8, 8, nz, 0.1, 0.1, 0.1, *wl.parse_bc(combo))
         assert (st == 0) == ok, (nz, combo, st)
         if h:
