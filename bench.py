@@ -2,7 +2,7 @@
 """Benchmark of the direct Poisson solve (BASELINE.json metric: Gpoints/s per fp64 Poisson solve and
 % of HBM roofline at 512x512x256).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg3|cfg4|cfg5|cfg2]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg3|cfg4|cfg5|cfg2|pencil] [--fusion]
 
 A "step" is one pp_solve: the whole hot path (x-fwd, y-fwd, z-solve, y-inv, x-inv) over one synthetic
 grid.  N > 1 runs N independent replicas (one process per GPU, no data-path collective -- DESIGN.md
@@ -42,6 +42,8 @@ def workload_by_name(name):
         return wl.config2("PPN", "normal")
     if name == "cfg1":
         return wl.config1("uniform")
+    if name == "pencil":
+        return wl.paper_pencil("PPN")
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -249,6 +251,9 @@ def run_cuda(args):
     nz, ny, nx = w.shape
     npts = w.n_points
     plan = pp.Plan(nx, ny, nz, *w.h, w.bc)
+    if args.fusion:
+        plan.set_xy_fusion(True)
+    launches = plan.launches_per_solve
     f = torch.from_numpy(w.f).cuda()
     u = torch.empty_like(f)
     stream = torch.cuda.current_stream()
@@ -301,8 +306,15 @@ def run_cuda(args):
 
     if rank == 0:
         peak, peak_src = measured_peak()
-        dom = max(kernel_ms, key=kernel_ms.get)
-        achieved = BYTES_PER_POINT_KERNEL * npts / (kernel_ms[dom] * 1e-3) / 1e9
+        # algorithmic bytes per point of each timed slot: 16 per pass; with x+y fusion
+        # the pair's 32 sit in the x slot; the two-level z solve of long lines reads twice (24)
+        slot_bytes = dict.fromkeys(pp.KERNEL_NAMES, BYTES_PER_POINT_KERNEL)
+        if args.fusion:
+            slot_bytes.update(x_fwd=32.0, y_fwd=0.0, y_inv=0.0, x_inv=32.0)
+        if launches - (2 if args.fusion else 4) > 1:
+            slot_bytes["z_solve"] = 24.0
+        dom = max((k for k in kernel_ms if slot_bytes[k] > 0), key=lambda k: kernel_ms[k] / slot_bytes[k])
+        achieved = slot_bytes[dom] * npts / (kernel_ms[dom] * 1e-3) / 1e9
         solve_gbs = BYTES_PER_POINT_SOLVE * npts / (ms_step * 1e-3) / 1e9
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -310,19 +322,19 @@ def run_cuda(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": describe(w), "parallelism": f"replicas x{world} (no collective)",
                        "l2_policy": "inputs larger than L2 (f and u are %d MiB each)" % (npts * 8 >> 20),
-                       "in_place": False},
+                       "in_place": False, "xy_fusion": bool(args.fusion), "kernels_per_solve": launches},
             "clocks": sampler.result(),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": npts * 8, "d2h_bytes_per_step": npts * 8,
                     "ms_per_step": e2e_ms, "steps": e2e_steps, "api": "pp_solve_host (pinned host buffers)"},
-            "gpu_launches": 5 * args.steps,
+            "gpu_launches": launches * args.steps,
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "traffic": committed_traffic(dom), "peak_source": peak_src,
-                         "algorithmic_bytes_per_launch": BYTES_PER_POINT_KERNEL * npts},
+                         "algorithmic_bytes_per_launch": slot_bytes[dom] * npts},
             "roofline_solve": {"bound": "hbm", "achieved": solve_gbs, "peak": peak, "unit": "GB/s",
                                "frac": solve_gbs / peak, "bytes_per_point": BYTES_PER_POINT_SOLVE,
                                "frac_of_nominal_8TBs": solve_gbs / 8000.0},
             "kernel_ms": kernel_ms,
-            "kernel_gbs": {k: BYTES_PER_POINT_KERNEL * npts / (v * 1e-3) / 1e9 for k, v in kernel_ms.items()},
+            "kernel_gbs": {k: slot_bytes[k] * npts / (v * 1e-3) / 1e9 for k, v in kernel_ms.items() if slot_bytes[k] > 0},
         }
         if world == 1 and not args.no_cpu_baseline:
             sample = oracle_sample(w, step_seconds=18.0)
@@ -343,7 +355,8 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="cfg3", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--workload", default="cfg3", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "pencil"])
+    ap.add_argument("--fusion", action="store_true", help="plane-wise x+y fusion through L2 (opt-in, DESIGN.md)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

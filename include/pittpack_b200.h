@@ -140,6 +140,13 @@ int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm);
  */
 int pp_plan_set_xy_fusion(pp_plan *plan, int enable);
 
+/*
+ * Number of kernels one pp_solve launches with the plan's current settings: 5 by default (PP_K_*),
+ * 3 with x+y fusion, +2 (+1 more when the problem is singular) when the z solve is the two-level
+ * partition for long lines.  0 for a NULL plan.
+ */
+int pp_plan_launches_per_solve(const pp_plan *plan);
+
 /* Static, NUL-terminated description of a status code. */
 const char *pp_strerror(int status);
 

@@ -21,7 +21,7 @@ KERNEL_NAMES = ("x_fwd", "y_fwd", "z_solve", "y_inv", "x_inv")
 
 EXPORTS = (
     "pp_plan_create", "pp_solve", "pp_solve_host", "pp_plan_destroy", "pp_plan_workspace_bytes",
-    "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_plan_set_xy_fusion", "pp_strerror", "pp_version",
+    "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_plan_set_xy_fusion", "pp_plan_launches_per_solve", "pp_strerror", "pp_version",
 )
 PP_Z_AUTO, PP_Z_SWEEP, PP_Z_PARTITION = 0, 1, 2
 
@@ -63,6 +63,8 @@ def lib() -> ctypes.CDLL:
     L.pp_plan_set_z_algorithm.restype = i32
     L.pp_plan_set_xy_fusion.argtypes = [vp, i32]
     L.pp_plan_set_xy_fusion.restype = i32
+    L.pp_plan_launches_per_solve.argtypes = [vp]
+    L.pp_plan_launches_per_solve.restype = i32
     L.pp_strerror.argtypes = [i32]
     L.pp_strerror.restype = ctypes.c_char_p
     L.pp_version.argtypes = []
@@ -115,6 +117,10 @@ def pp_plan_set_z_algorithm(plan, algorithm):
 
 def pp_plan_set_xy_fusion(plan, enable):
     return lib().pp_plan_set_xy_fusion(ctypes.c_void_p(plan), int(bool(enable)))
+
+
+def pp_plan_launches_per_solve(plan):
+    return int(lib().pp_plan_launches_per_solve(ctypes.c_void_p(plan)))
 
 
 def strerror(status: int) -> str:
@@ -203,6 +209,10 @@ class Plan:
         st = pp_plan_set_xy_fusion(self.handle, enable)
         if st != PP_SUCCESS:
             raise PittPackError(st, "pp_plan_set_xy_fusion")
+
+    @property
+    def launches_per_solve(self):
+        return pp_plan_launches_per_solve(self.handle)
 
     @property
     def workspace_bytes(self):

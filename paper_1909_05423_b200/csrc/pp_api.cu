@@ -481,6 +481,16 @@ int pp_plan_set_xy_fusion(pp_plan *plan, int enable) {
     return PP_SUCCESS;
 }
 
+int pp_plan_launches_per_solve(const pp_plan *plan) {
+    if (!plan) return 0;
+    const bool fused = plan->xy_fusion && fusion_supported(plan->nx, plan->ny);
+    int n = fused ? 2 : 4;                                        // x/y passes
+    const bool want_part = plan->bcz != PP_BC_PERIODIC && plan->z_algorithm != PP_Z_SWEEP;
+    if (want_part && zpart_shape(plan->nz).R == 0 && plan->hier_scratch) n += 3 + (plan->singular ? 1 : 0);
+    else n += 1;
+    return n;
+}
+
 int pp_plan_last_kernel_ms(pp_plan *plan, float *ms_out) {
     if (!plan || !ms_out) return PP_ERR_NULL;
     if (!plan->have_times) return PP_ERR_INVALID_ARG;
