@@ -24,6 +24,10 @@
 
 namespace pp {
 
+#ifndef PP_FUSE_LDCG
+#define PP_FUSE_LDCG true   // second-phase tiles read with ld.global.cg (L2): their input comes from other SMs
+#endif
+
 struct FusedParams {
     int nz, nxh;            // planes, double2 per row
     int na, nb;             // first-/second-phase tasks per plane
@@ -57,6 +61,29 @@ __device__ __forceinline__ int ld_acquire_gpu(const int *p) {
     return v;
 }
 
+// The four tile bodies as real (not inlined) functions: each gets its own register allocation, and
+// nothing of the scheduler's state is live inside them.
+template <int N, int TX>
+__device__ __noinline__ void fused_xfwd(const double *in, double *u, long long pair0, long long pend, int bc,
+                                        const double2 *tw, const double2 *ptw, double2 *smem) {
+    xfwd_tile<N, TX>(in, u, pair0, pend, bc, tw, ptw, smem);
+}
+template <int N, int TX>
+__device__ __noinline__ void fused_xinv(double *u, long long pair0, long long pend, int bc,
+                                        const double2 *tw, const double2 *ptw, double2 *smem) {
+    xinv_tile<N, TX, PP_FUSE_LDCG>(u, u, pair0, pend, bc, tw, ptw, smem);
+}
+template <int N>
+__device__ __noinline__ void fused_yfwd(double2 *u, int nxh, int bc, int cc, const double2 *tw, const double2 *ptw,
+                                        int bx, int z, double2 *smem) {
+    yfwd_tile<N, PP_FUSE_LDCG>(u, nxh, bc, cc, tw, ptw, bx, z, smem);
+}
+template <int N>
+__device__ __noinline__ void fused_yinv(double2 *u, int nxh, int bc, int cc, const double2 *tw, const double2 *ptw,
+                                        int bx, int z, double2 *smem) {
+    yinv_tile<N>(u, nxh, bc, cc, tw, ptw, bx, z, smem);
+}
+
 // FWD_DIR: x forward tiles then y forward tiles (in -> u, then in place);
 // otherwise y inverse tiles then x inverse tiles (in place in u).
 template <int N, bool FWD_DIR>
@@ -88,11 +115,11 @@ xy_fused_kernel(const double *in, double *u, FusedParams p,
         if (xtile) {
             const long long pair0 = (long long)k.z * p.pairs_per_plane + (long long)k.idx * TX;
             const long long pend = (long long)(k.z + 1) * p.pairs_per_plane;     // tiles do not straddle planes
-            if (FWD_DIR) xfwd_tile<N, TX>(in, u, pair0, pend, p.bcx, tw_x, ptw_x, smem);
-            else         xinv_tile<N, TX, true>(u, u, pair0, pend, p.bcx, tw_x, ptw_x, smem);
+            if (FWD_DIR) fused_xfwd<N, TX>(in, u, pair0, pend, p.bcx, tw_x, ptw_x, smem);
+            else         fused_xinv<N, TX>(u, pair0, pend, p.bcx, tw_x, ptw_x, smem);
         } else {
-            if (FWD_DIR) yfwd_tile<N, true>((double2 *)u, p.nxh, p.bcy, p.complex_cols, tw_y, ptw_y, k.idx, k.z, smem);
-            else         yinv_tile<N>((double2 *)u, p.nxh, p.bcy, p.complex_cols, tw_y, ptw_y, k.idx, k.z, smem);
+            if (FWD_DIR) fused_yfwd<N>((double2 *)u, p.nxh, p.bcy, p.complex_cols, tw_y, ptw_y, k.idx, k.z, smem);
+            else         fused_yinv<N>((double2 *)u, p.nxh, p.bcy, p.complex_cols, tw_y, ptw_y, k.idx, k.z, smem);
         }
         __syncthreads();                                // the tile is done with smem; its stores are issued
         if (threadIdx.x == 0) {
