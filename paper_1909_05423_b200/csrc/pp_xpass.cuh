@@ -199,55 +199,71 @@ __device__ __forceinline__ void xinv_tile(const double *in, double *out, long lo
                 s[lay(N - m)] = make_double2(A.x + B.y, B.x - A.y);    // Z_{N-m}
             }
         }
-        sync();
+    } else {
+        // Neumann / Dirichlet: V_m = conj(w_m) (Y_m - i Y_{N-m}) and V_{N-m} = conj(w_{N-m}) (Y_{N-m} - i Y_m)
+        // need the same two coefficients, and conj(w_{N-m}) = i w_m.  The owner of m in [0, N/2) loads the
+        // pair once, keeps V_m and hands V_{N-m} to its owner through shared memory, exactly as above.
+        // Packed rows: Y = Ya + i Yb, so Y_m - i Y_{N-m} = (ya + ybp) + i (yb - yap).
 #pragma unroll
-        for (int q = E / 2; q < E; ++q) v[q] = s[lay(t + q * P)];
-        sync();
-    }
-#pragma unroll
-    for (int q = 0; q < E; ++q) {
-        const int m = t + q * P;
-        if (bc == BC_P) {
-        } else {
-            double ya, yb, yap, ybp;
+        for (int q = 0; q < E / 2; ++q) {
+            const int m = t + q * P;
+            double ya, yb, yap = 0.0, ybp = 0.0;
             if (bc == BC_N) {
                 ya = xld<LDCG>(ra + m); yb = xld<LDCG>(rb + m);
-                yap = (m == 0) ? 0.0 : xld<LDCG>(ra + N - m);
-                ybp = (m == 0) ? 0.0 : xld<LDCG>(rb + N - m);
+                if (m > 0) { yap = xld<LDCG>(ra + N - m); ybp = xld<LDCG>(rb + N - m); }
             } else {                                                   // Y'_m = (-1)^m S_{N-1-m}
                 const double s1 = sgn_of(m);
                 ya = s1 * xld<LDCG>(ra + N - 1 - m); yb = s1 * xld<LDCG>(rb + N - 1 - m);
-                yap = (m == 0) ? 0.0 : s1 * xld<LDCG>(ra + m - 1);                 // (-1)^(N-m) S_{m-1}
-                ybp = (m == 0) ? 0.0 : s1 * xld<LDCG>(rb + m - 1);
+                if (m > 0) { yap = s1 * xld<LDCG>(ra + m - 1); ybp = s1 * xld<LDCG>(rb + m - 1); }   // (-1)^(N-m) S_{m-1}
             }
-            const double2 w = cconj(__ldg(&ptw[m]));
-            v[q] = cmul(w, make_double2(ya + ybp, yb - yap));          // conj(w)^m (Y_m - i Y_{N-m})
+            const double2 w = __ldg(&ptw[m]);
+            v[q] = cmul(cconj(w), make_double2(ya + ybp, yb - yap));
+            if (m > 0) {
+                s[lay(N - m)] = cmul(make_double2(w.y * -1.0, w.x), make_double2(yap + yb, ybp - ya));   // i w_m (...)
+            } else {                                                   // thread 0 also makes V_{N/2} (its own partner)
+                double ha, hb;
+                if (bc == BC_N) { ha = xld<LDCG>(ra + H); hb = xld<LDCG>(rb + H); }
+                else { const double sh = sgn_of(H); ha = sh * xld<LDCG>(ra + N - 1 - H); hb = sh * xld<LDCG>(rb + N - 1 - H); }
+                s[lay(H)] = cmul(cconj(__ldg(&ptw[H])), make_double2(ha + hb, hb - ha));
+            }
         }
     }
-    // all loads of this row pair are done before any thread of the group stores (in-place safe):
-    // the FFT's exchanges synchronise the group; for single-stage transforms sync explicitly
-    if constexpr (C::R0 == N) { if (bc != BC_P) sync(); }
+    // every load of this row pair precedes the barrier, every store follows it: in-place safe
+    sync();
+#pragma unroll
+    for (int q = E / 2; q < E; ++q) v[q] = s[lay(t + q * P)];
+    sync();
 
     fft<N, INV>(v, t, s, tw, lay, sync);
 
+    if (bc == BC_P) {
+        if (active) {
+#pragma unroll
+            for (int q = 0; q < E; ++q) { oa[t + q * P] = v[q].x; ob[t + q * P] = v[q].y; }
+        }
+        return;
+    }
+    // Neumann / Dirichlet: the un-permutation sends v_i to position 2i and v_{N-1-i} to
+    // 2i+1 (i < N/2) -- neighbours.  The upper half goes through shared memory to the owner of i, which
+    // stores both as one 16-byte element instead of two 8-byte ones at stride 2.
+#pragma unroll
+    for (int q = E / 2; q < E; ++q) s[lay(t + q * P)] = v[q];
+    sync();
     if (active) {
 #pragma unroll
-        for (int q = 0; q < E; ++q) {
-            const int i = t + q * P;
-            if (bc == BC_P) {
-                oa[i] = v[q].x; ob[i] = v[q].y;
-            } else {
-                const int p = (i < H) ? 2 * i : 2 * (N - 1 - i) + 1;   // un-permute
-                if (bc == BC_N) { oa[p] = v[q].x; ob[p] = v[q].y; }
-                else {                                                 // x_{N-1-p} = -(-1)^p x'_p
-                    const double s1 = -sgn_of(p);
-                    oa[N - 1 - p] = s1 * v[q].x; ob[N - 1 - p] = s1 * v[q].y;
-                }
+        for (int q = 0; q < E / 2; ++q) {
+            const int i = t + q * P;                                   // 0 <= i < N/2
+            const double2 lo = v[q], hi = s[lay(N - 1 - i)];
+            if (bc == BC_N) {
+                *reinterpret_cast<double2 *>(oa + 2 * i) = make_double2(lo.x, hi.x);
+                *reinterpret_cast<double2 *>(ob + 2 * i) = make_double2(lo.y, hi.y);
+            } else {                                                   // x_{N-1-p} = -(-1)^p x'_p: (x_{N-2-2i}, x_{N-1-2i})
+                *reinterpret_cast<double2 *>(oa + N - 2 - 2 * i) = make_double2(hi.x, -lo.x);
+                *reinterpret_cast<double2 *>(ob + N - 2 - 2 * i) = make_double2(hi.y, -lo.y);
             }
         }
     }
 }
-
 
 template <int N>
 __global__ void __launch_bounds__(XCfg<N>::THREADS, PP_X_MINB)

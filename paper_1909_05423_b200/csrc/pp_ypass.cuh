@@ -173,37 +173,58 @@ __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int compl
     const bool cplx = complex_cols && cp > 0;
 
     double2 v[E];
+    if (complex_cols && bx > 0) {                          // block-uniform: every column of the tile is complex
 #pragma unroll
-    for (int q = 0; q < E; ++q) {
-        const int m = t + q * P;
-        if (cplx) {
-            v[q] = base[m * ld];
-        } else if (bc == BC_P) {
-            if (m == 0 || m == H) {
-                v[q] = base[m * ld];                                   // (A, B) both real: Z = A + i B
-            } else if (m < H) {
-                const double2 lo = base[m * ld], hi = base[(N - m) * ld];
-                v[q] = make_double2(lo.x - hi.y, hi.x + lo.y);
+        for (int q = 0; q < E; ++q) v[q] = base[(t + q * P) * ld];
+    } else {
+        // Real pairs: row m and row N-m are needed together, for V_m and for V_{N-m}.  The owner of
+        // m in [0, N/2) loads the two rows once, keeps V_m and hands V_{N-m} to its owner through shared
+        // memory (thread 0 also makes V_{N/2}).  A complex column inside such a tile (periodic x and y,
+        // first tile) just loads its eight rows and takes part in the barriers.
+#pragma unroll
+        for (int q = 0; q < E / 2; ++q) {
+            const int m = t + q * P;                       // 0 <= m < N/2
+            if (cplx) {
+                v[q] = base[m * ld];
+                v[q + E / 2] = base[(m + H) * ld];
+            } else if (bc == BC_P) {
+                if (m == 0) {                              // (A, B) both real: Z = A + i B
+                    v[q] = base[0];
+                    smem[lay(H)] = base[H * ld];
+                } else {
+                    const double2 lo = base[m * ld], hi = base[(N - m) * ld];
+                    v[q] = make_double2(lo.x - hi.y, hi.x + lo.y);
+                    smem[lay(N - m)] = make_double2(lo.x + hi.y, lo.y - hi.x);
+                }
             } else {
-                const double2 lo = base[(N - m) * ld], hi = base[m * ld];
-                v[q] = make_double2(lo.x + hi.y, lo.y - hi.x);
+                double2 ym, yp = make_double2(0.0, 0.0);
+                if (bc == BC_N) {
+                    ym = base[m * ld];
+                    if (m > 0) yp = base[(N - m) * ld];
+                } else {
+                    const double s1 = sgn_of(m);
+                    ym = dscale(s1, base[(N - 1 - m) * ld]);
+                    if (m > 0) yp = dscale(s1, base[(m - 1) * ld]);
+                }
+                const double2 wm = __ldg(&ptw[m]);
+                v[q] = cmul(cconj(wm), make_double2(ym.x + yp.y, ym.y - yp.x));
+                if (m > 0) {                               // conj(w_{N-m}) = i w_m
+                    smem[lay(N - m)] = cmul(make_double2(-wm.y, wm.x), make_double2(yp.x + ym.y, yp.y - ym.x));
+                } else {
+                    const double2 yh = (bc == BC_N) ? base[H * ld] : dscale(sgn_of(H), base[(N - 1 - H) * ld]);
+                    smem[lay(H)] = cmul(cconj(__ldg(&ptw[H])), make_double2(yh.x + yh.y, yh.y - yh.x));
+                }
             }
-        } else {
-            double2 ym, yp;
-            if (bc == BC_N) {
-                ym = base[m * ld];
-                yp = (m == 0) ? make_double2(0.0, 0.0) : base[(N - m) * ld];
-            } else {
-                const double s1 = sgn_of(m);
-                ym = dscale(s1, base[(N - 1 - m) * ld]);
-                yp = (m == 0) ? make_double2(0.0, 0.0) : dscale(s1, base[(m - 1) * ld]);
-            }
-            const double2 wm = cconj(__ldg(&ptw[m]));
-            v[q] = cmul(wm, make_double2(ym.x + yp.y, ym.y - yp.x));
         }
+        sync();
+        if (!cplx) {
+#pragma unroll
+            for (int q = E / 2; q < E; ++q) v[q] = smem[lay(t + q * P)];
+        }
+        sync();
     }
-    // in place: every load of the tile precedes every store -- the FFT's exchanges are CTA-wide
-    // barriers; a single-stage transform has P = 1 (one thread owns the whole column)
+    // in place: every load of the tile precedes every store -- the barriers above and the FFT's
+    // exchanges are CTA-wide; a single-stage transform has P = 1 (one thread owns the whole column)
 
     fft<N, INV>(v, t, smem, tw, lay, sync);
 
