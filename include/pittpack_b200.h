@@ -114,14 +114,15 @@ int pp_plan_last_kernel_ms(pp_plan *plan, float *ms_out);
  * tridiagonal algorithm open and offers several).  Both compute the same
  * Thomas elimination of Algorithm 2 up to rounding order.
  *   PP_Z_AUTO      : partitioned where it applies, two-sweep otherwise (the default).
- *   PP_Z_SWEEP     : two-sweep Thomas, one thread per system, any nz; periodic z always uses it
- *                    (Sherman-Morrison).
+ *   PP_Z_SWEEP     : two-sweep Thomas, one thread per system, any nz <= 4096; periodic z by
+ *                    Sherman-Morrison.
  *   PP_Z_PARTITION : each system cut into segments of 32 or 64 rows held in registers and
  *                    coupled through their interface unknowns (the reduction idea of CR-P,
- *                    PAPER.md:250-258, across the threads of one CTA).  Needs Neumann or
- *                    Dirichlet z and nz = 32 m or 64 m (m <= 8), 1024 or 2048 -- or nz = 256 m
- *                    (2 <= m <= 64), where the same partition is applied on two levels
- *                    (super-segments of 256 rows, three kernels); otherwise
+ *                    PAPER.md:250-258, across the threads of one CTA); with periodic z the
+ *                    interface chain closes on itself (a 2x2 closure instead of Sherman-Morrison's
+ *                    second solve).  Needs nz = 32 m or 64 m (m <= 8), 1024 or 2048 -- or, for
+ *                    Neumann / Dirichlet z, nz = 256 m (2 <= m <= 64), where the same partition is
+ *                    applied on two levels (super-segments of 256 rows, three kernels); otherwise
  *                    PP_ERR_UNSUPPORTED_SIZE and the plan is left unchanged.  PP_Z_SWEEP is
  *                    refused for nz > 4096.
  */

@@ -231,20 +231,23 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
 #ifndef PP_Z_CB
 #define PP_Z_CB 16
 #endif
-    const bool want_part = p->bcz != PP_BC_PERIODIC && p->z_algorithm != PP_Z_SWEEP;
+    const bool want_part = p->z_algorithm != PP_Z_SWEEP;
     const ZPartShape zs = want_part ? zpart_shape(p->nz) : ZPartShape{0, 0, 0};
     if (zs.R) {
         // partitioned, register-resident solve: one HBM read + one write per unknown (pp_zpart.cuh)
-        const size_t ds = zpart_smem_bytes(zs);
+        const bool cyc = p->bcz == PP_BC_PERIODIC;
+        const size_t ds = zpart_smem_bytes(zs, cyc);
         const unsigned grid = (unsigned)((plane + zs.L - 1) / zs.L);
         const ZHier none = {1, nullptr, nullptr};
-        if (zs.R == 32) {
-            if (int rc = set_smem(zsolve_part_kernel<32, 0>, ds)) return rc;
-            zsolve_part_kernel<32, 0><<<grid, zs.L * zs.S, ds, st>>>(w, zp, zs.S, zs.L, none);
-        } else {
-            if (int rc = set_smem(zsolve_part_kernel<64, 0>, ds)) return rc;
-            zsolve_part_kernel<64, 0><<<grid, zs.L * zs.S, ds, st>>>(w, zp, zs.S, zs.L, none);
-        }
+        auto launch = [&](auto kernel) -> int {
+            if (int rc = set_smem(kernel, ds)) return rc;
+            kernel<<<grid, zs.L * zs.S, ds, st>>>(w, zp, zs.S, zs.L, none);
+            return PP_SUCCESS;
+        };
+        int rc;
+        if (zs.R == 32) rc = cyc ? launch(zsolve_part_kernel<32, 0, true>) : launch(zsolve_part_kernel<32, 0, false>);
+        else            rc = cyc ? launch(zsolve_part_kernel<64, 0, true>) : launch(zsolve_part_kernel<64, 0, false>);
+        if (rc) return rc;
     } else if (want_part && p->hier_scratch) {
         // long lines: two-level partition, 8 + 16 bytes per unknown (pp_zpart.cuh, ZHier)
         const ZPartShape hs = {32, ZP_HIER_ROWS / 32, 32};
@@ -467,7 +470,7 @@ int pp_plan_set_profiling(pp_plan *plan, int enable) {
 int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm) {
     if (!plan) return PP_ERR_NULL;
     if (algorithm != PP_Z_AUTO && algorithm != PP_Z_SWEEP && algorithm != PP_Z_PARTITION) return PP_ERR_INVALID_ARG;
-    if (algorithm == PP_Z_PARTITION && (plan->bcz == PP_BC_PERIODIC || (zpart_shape(plan->nz).R == 0 && !plan->hier_scratch)))
+    if (algorithm == PP_Z_PARTITION && zpart_shape(plan->nz).R == 0 && !plan->hier_scratch)
         return PP_ERR_UNSUPPORTED_SIZE;
     if (algorithm == PP_Z_SWEEP && plan->nz > 64 * Z_MAX_CK) return PP_ERR_UNSUPPORTED_SIZE;
     plan->z_algorithm = algorithm;
@@ -485,7 +488,7 @@ int pp_plan_launches_per_solve(const pp_plan *plan) {
     if (!plan) return 0;
     const bool fused = plan->xy_fusion && fusion_supported(plan->nx, plan->ny);
     int n = fused ? 2 : 4;                                        // x/y passes
-    const bool want_part = plan->bcz != PP_BC_PERIODIC && plan->z_algorithm != PP_Z_SWEEP;
+    const bool want_part = plan->z_algorithm != PP_Z_SWEEP;
     if (want_part && zpart_shape(plan->nz).R == 0 && plan->hier_scratch) n += 3 + (plan->singular ? 1 : 0);
     else n += 1;
     return n;

@@ -68,8 +68,10 @@ inline bool zpart_hier_ok(int nz) { return nz % ZP_HIER_ROWS == 0 && nz / ZP_HIE
 //   F [6][S][L]     factored interface matrix (right-hand-side independent): vL, vF, D, A D, sc, sa
 //   PC, PA [S][L]   right-hand-side part of the interface elimination
 //   RQ [2][L]       1 / q_R of the two blocks
-inline size_t zpart_smem_bytes(const ZPartShape &z) {
-    return sizeof(double) * (size_t)z.L * (2 * (z.R + 1) + 2 * z.R + 10 * z.S + 2);
+//   ZC [4][S][L]    periodic z only: the interface chain's responses to its two wrap-around couplings
+//   CL [4][L]       periodic z only: b1 times the inverse of the 2x2 closure matrix
+inline size_t zpart_smem_bytes(const ZPartShape &z, bool periodic = false) {
+    return sizeof(double) * (size_t)z.L * (2 * (z.R + 1) + 2 * z.R + 10 * z.S + 2 + (periodic ? 4 * z.S + 4 : 0));
 }
 
 // keeps the compiler from hoisting a whole unrolled loop's shared-memory loads above it (which
@@ -109,9 +111,10 @@ struct ZHier {
     double *HF, *HL;         // [nK][plane]
 };
 
-template <int R, int MODE>
+template <int R, int MODE, bool CYC = false>
 __global__ void __launch_bounds__(PP_ZP_MAXT, (R == 32) ? PP_ZP_MINB : PP_ZP_MINB / 2)
 zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
+    static_assert(!CYC || MODE == 0, "periodic z: single-level only");
     static_assert(R % 2 == 0, "the spike signs below assume an even segment length");
     extern __shared__ double zsm[];
     double *Q = zsm;                                  // [2][R+1][L]
@@ -121,7 +124,13 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
     double *F = YL + S * L;                           // [6][S][L]
     double *PC = F + 6 * S * L, *PA = PC + S * L;
     double *RQ = PA + S * L;                          // [2][L]
+    double *ZC = RQ + 2 * L;                          // [4][S][L]
+    double *CL = ZC + 4 * S * L;                      // [4][L]
     const int SL = S * L;
+    // Periodic z: every segment is an interior block and the interface chain closes on itself
+    // (S interfaces instead of S - 1); see the closure below.
+    constexpr bool cyc = CYC;
+    const int NI = cyc ? S : S - 1;                   // interfaces
 
     const int l = threadIdx.x % L, j = threadIdx.x / L;
     const size_t plane = (size_t)p.nx * p.ny;
@@ -129,8 +138,8 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
     const bool live = e < plane;
     const bool pin = !live || (p.singular && e == 0);       // pinned line: computed with a placeholder, never stored
     const int K = (MODE == 0) ? 0 : (int)blockIdx.y;         // super-segment of this CTA
-    const bool top_end = (MODE == 0) || K == 0;               // the CTA's rows start at the line's first row
-    const bool bot_end = (MODE == 0) || K == h.nK - 1;        // ... end at its last row
+    const bool top_end = !cyc && ((MODE == 0) || K == 0);          // the CTA's rows start at the line's first row
+    const bool bot_end = !cyc && ((MODE == 0) || K == h.nK - 1);   // ... end at its last row
     const bool mirror = bot_end && (S > 1) && (j == S - 1);   // line's last segment: rows held in reverse order
     const int c = ((j == 0 && top_end) || (j == S - 1 && bot_end)) ? 0 : 1;   // first (and mirrored last) / interior block
     // row i of the segment lives at row0 + i * step (the mirrored segment walks upwards)
@@ -139,7 +148,8 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
 
     // the mode's shift first (the tabulating threads start from it), then every right-hand side of
     // the segment, in flight at once
-    const int jfac = (S >= 3) ? 2 : 1;
+    const int jint = cyc ? 0 : 1;                             // who tabulates the interior block
+    const int jfac = cyc ? ((S >= 2) ? 1 : 0) : ((S >= 3) ? 2 : 1);   // who factors the interface matrix
     double s = -1.0;
     if (j <= jfac && !pin) s = __ldg(p.sx + (int)(e % p.nx)) + __ldg(p.sy + (int)(e / p.nx));
     double ext0 = 0.0, ext1 = 0.0;                            // x just above the CTA's first row / below its last
@@ -157,10 +167,10 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
         const double bint = -2.0 + s;
         const double bend = ((p.bcz == 1) ? -1.0 : -3.0) + s;
         double qa, qb;
-        if (j == 0) {
+        if (j == 0 && !cyc) {
             zp_minors<R, true>(bend, bint, (S == 1) ? bend : bint, Q + l, G + l, L, qa, qb);
             RQ[l] = fast_rcp(qb);
-        } else if (j == 1) {
+        } else if (j == jint) {
             zp_minors<R, true>(bint, bint, bint, Q + (R + 1) * L + l, G + R * L + l, L, qa, qb);
             RQ[L + l] = fast_rcp(qb);
         }
@@ -182,7 +192,8 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
                 im = ic; ic = in;
             }
             const double rqe = fast_rcp(ec), rqi = fast_rcp(ic);
-            const double a1 = (S >= 3 || MODE != 0) ? im * rqi : 0.0, b1 = (S >= 3 || MODE != 0) ? -rqi : 0.0;
+            const bool interior = S >= 3 || MODE != 0 || cyc;                  // is there an interior-type block at all
+            const double a1 = interior ? im * rqi : 0.0, b1 = interior ? -rqi : 0.0;
             const double a0 = em * rqe;
             const double atop = top_end ? a0 : a1, abot = bot_end ? a0 : a1;
             // A_J obeys the Moebius recurrence A_0 = a0, A_J = a1 + b1^2 A_{J-1} / (1 - a1 A_{J-1}); carried
@@ -190,9 +201,9 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
             //   D_J = M_J / (M_J - vF_J N_J),   (A D)_J = N_J / (M_J - vF_J N_J)
             const double k1 = fma(b1, b1, -a1 * a1);
             double N = atop, M = 1.0;
-            for (int J = 0; J < S - 1; ++J) {
+            for (int J = 0; J < NI; ++J) {
                 const double vL = (J == 0) ? 0.0 : b1;
-                const double vF = (J + 1 == S - 1) ? abot : a1, wF = (J + 1 == S - 1) ? 0.0 : b1;
+                const double vF = (J == NI - 1) ? abot : a1, wF = (J == NI - 1) ? 0.0 : b1;
                 const double r = fast_rcp(fma(-vF, N, M));
                 const double D = M * r, AD = N * r;
                 double *f = F + J * L + l;
@@ -200,6 +211,41 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
                 const double Nn = fma(k1, N, a1 * M), Mn = fma(-a1, N, M);
                 N = Nn;
                 M = Mn;
+            }
+            if (cyc) {
+                // Closure of the periodic chain.  The full interface matrix is the open chain plus the two
+                // wrap-around couplings  b1 a_{S-1} in row a_0  and  b1 c_0 in row c_{S-1}:
+                //   x = x0 - (b1 a_{S-1}) z1 - (b1 c_0) z2,   z1 = chain^-1 e(row a_0),  z2 = chain^-1 e(row c_{S-1}),
+                // and the two wrapped unknowns follow from the 2x2 system  K (a_{S-1}, c_0)^T = (x0a_{S-1}, x0c_0)^T,
+                //   K = [1 + b1 z1a_{S-1},  b1 z2a_{S-1};  b1 z1c_0,  1 + b1 z2c_0].
+                // z1, z2 depend on the mode only: solved here with the factors just stored.
+                double *z1c = ZC + l, *z1a = z1c + SL, *z2c = z1a + SL, *z2a = z2c + SL;
+                double pa1 = 0.0;
+                for (int J = 0; J < S; ++J) {                   // forward, both unit right-hand sides
+                    const double *f = F + J * L + l;
+                    const double Ya = fma(-f[0], pa1, (J == 0) ? 1.0 : 0.0);
+                    const double t1 = -f[SL] * Ya;
+                    pa1 = fma(-f[3 * SL], t1, Ya);
+                    z1c[J * L] = f[2 * SL] * t1;
+                    z1a[J * L] = pa1;
+                    z2c[J * L] = (J == S - 1) ? f[2 * SL] : 0.0;
+                    z2a[J * L] = (J == S - 1) ? -f[3 * SL] : 0.0;
+                }
+                double c1 = 0.0, c2 = 0.0;
+                for (int J = S - 1; J >= 0; --J) {              // backward
+                    const double *f = F + J * L + l;
+                    const double sc = f[4 * SL], sa = f[5 * SL];
+                    z1a[J * L] = fma(-sa, c1, z1a[J * L]);
+                    c1 = fma(-sc, c1, z1c[J * L]);
+                    z1c[J * L] = c1;
+                    z2a[J * L] = fma(-sa, c2, z2a[J * L]);
+                    c2 = fma(-sc, c2, z2c[J * L]);
+                    z2c[J * L] = c2;
+                }
+                const double k11 = fma(b1, z1a[(S - 1) * L], 1.0), k12 = b1 * z2a[(S - 1) * L];
+                const double k21 = b1 * z1c[0], k22 = fma(b1, z2c[0], 1.0);
+                const double rdet = b1 / fma(k11, k22, -k12 * k21);
+                CL[l] = k22 * rdet; CL[L + l] = -k12 * rdet; CL[2 * L + l] = -k21 * rdet; CL[3 * L + l] = k11 * rdet;
             }
         }
     }
@@ -212,7 +258,7 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
     {
         constexpr int M = R / 2;
         const double *gt = G + c * R * L + l;
-        const double *gb = G + ((S == 1) ? 0 : R * L) + l;
+        const double *gb = G + ((S == 1 && !cyc) ? 0 : R * L) + l;
         const double scale = p.scale;
         y[0] = fma(y[0], scale, -ext0) * gt[0];
         y[R - 1] = fma(y[R - 1], scale, -ext1) * gb[0];
@@ -236,20 +282,22 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
         }
     }
 
-    if (S > 1) {
+    if (S > 1 || cyc) {
         YF[j * L + l] = mirror ? y[R - 1] : y[0];
         YL[j * L + l] = mirror ? y[0] : y[R - 1];
         __syncthreads();
         if (j == 0) {                                   // right-hand-side part of the interface elimination
-            // (the next step's coefficients are fetched before the current step's FMA chain)
+            // interface J couples the last row of segment J with the first row of segment JF(J) = J + 1
+            // (periodic: modulo S).  The next step's coefficients are fetched before the current step's FMA chain.
             const double *f = F + l;
-            double vL = f[0], vF = f[SL], D = f[2 * SL], A = f[3 * SL], yl = YL[l], yf = YF[L + l];
+            double vL = f[0], vF = f[SL], D = f[2 * SL], A = f[3 * SL], yl = YL[l], yf = YF[((S > 1) ? L : 0) + l];
             double pa = 0.0;
-            for (int J = 0; J < S - 1; ++J) {
-                const int Jn = (J + 1 < S - 1) ? J + 1 : J;
+            for (int J = 0; J < NI; ++J) {
+                const int Jn = (J + 1 < NI) ? J + 1 : J;
+                const int JFn = (Jn + 1 < S) ? Jn + 1 : 0;
                 const double *fn = F + Jn * L + l;
                 const double nvL = fn[0], nvF = fn[SL], nD = fn[2 * SL], nA = fn[3 * SL];
-                const double nyl = YL[Jn * L + l], nyf = YF[(Jn + 1) * L + l];
+                const double nyl = YL[Jn * L + l], nyf = YF[JFn * L + l];
                 const double Ya = fma(-vL, pa, yl);
                 const double t = fma(-vF, Ya, yf);
                 const double pc = D * t;
@@ -258,25 +306,47 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
                 PA[J * L + l] = pa;
                 vL = nvL; vF = nvF; D = nD; A = nA; yl = nyl; yf = nyf;
             }
-            f = F + (S - 2) * L + l;
-            double sc = f[4 * SL], sa = f[5 * SL], pc = PC[(S - 2) * L + l], pav = PA[(S - 2) * L + l];
+            f = F + (NI - 1) * L + l;
+            double sc = f[4 * SL], sa = f[5 * SL], pc = PC[(NI - 1) * L + l], pav = PA[(NI - 1) * L + l];
             double cn = 0.0;
-            for (int J = S - 2; J >= 0; --J) {
-                const int Jn = (J > 0) ? J - 1 : 0;
-                const double *fn = F + Jn * L + l;
-                const double nsc = fn[4 * SL], nsa = fn[5 * SL], npc = PC[Jn * L + l], npa = PA[Jn * L + l];
-                const double cv = fma(-sc, cn, pc);
-                const double av = fma(-sa, cn, pav);
-                YL[J * L + l] = cv;                  // XR of segment J   = first row of segment J+1
-                YF[(J + 1) * L + l] = av;            // XL of segment J+1 = last row of segment J
-                cn = cv;
-                sc = nsc; sa = nsa; pc = npc; pav = npa;
+            if (!cyc) {
+                for (int J = NI - 1; J >= 0; --J) {
+                    const int Jn = (J > 0) ? J - 1 : 0;
+                    const double *fn = F + Jn * L + l;
+                    const double nsc = fn[4 * SL], nsa = fn[5 * SL], npc = PC[Jn * L + l], npa = PA[Jn * L + l];
+                    const double cv = fma(-sc, cn, pc);
+                    const double av = fma(-sa, cn, pav);
+                    YL[J * L + l] = cv;                  // XR of segment J   = first row of segment J+1
+                    YF[(J + 1) * L + l] = av;            // XL of segment J+1 = last row of segment J
+                    cn = cv;
+                    sc = nsc; sa = nsa; pc = npc; pav = npa;
+                }
+            } else {
+                // open-chain solution first (kept in PC, PA), then the closure: x = x0 - (b1 a_{S-1}) z1 - (b1 c_0) z2
+                for (int J = NI - 1; J >= 0; --J) {
+                    const int Jn = (J > 0) ? J - 1 : 0;
+                    const double *fn = F + Jn * L + l;
+                    const double nsc = fn[4 * SL], nsa = fn[5 * SL], npc = PC[Jn * L + l], npa = PA[Jn * L + l];
+                    const double cv = fma(-sc, cn, pc);
+                    PA[J * L + l] = fma(-sa, cn, pav);
+                    PC[J * L + l] = cv;
+                    cn = cv;
+                    sc = nsc; sa = nsa; pc = npc; pav = npa;
+                }
+                const double x0a = PA[(S - 1) * L + l], x0c = PC[l];
+                const double ba = fma(CL[l], x0a, CL[L + l] * x0c), bg = fma(CL[2 * L + l], x0a, CL[3 * L + l] * x0c);
+                const double *z1c = ZC + l, *z1a = z1c + SL, *z2c = z1a + SL, *z2a = z2c + SL;
+                for (int J = 0; J < S; ++J) {
+                    const int JF = (J + 1 < S) ? J + 1 : 0;
+                    YL[J * L + l] = fma(-ba, z1c[J * L], fma(-bg, z2c[J * L], PC[J * L + l]));    // XR of segment J
+                    YF[JF * L + l] = fma(-ba, z1a[J * L], fma(-bg, z2a[J * L], PA[J * L + l]));   // XL of segment JF
+                }
             }
         }
         __syncthreads();
         const double *qc = Q + c * (R + 1) * L + l;
-        const double xlg = (j >= 1) ? YF[j * L + l] : 0.0;
-        const double xrg = (j <= S - 2) ? YL[j * L + l] : 0.0;
+        const double xlg = (j >= 1 || cyc) ? YF[j * L + l] : 0.0;
+        const double xrg = (j <= S - 2 || cyc) ? YL[j * L + l] : 0.0;
         const double rq = RQ[c * L + l];
         const double XL = (c == 0) ? 0.0 : xlg * rq;
         const double XR = ((c == 0 && mirror) ? xlg : xrg) * rq;

@@ -15,7 +15,7 @@ PART_NZ = [32, 64, 96, 128, 160, 192, 224, 256, 320, 384, 448, 512, 1024, 2048]
 
 
 @pytest.mark.parametrize("nz", PART_NZ)
-@pytest.mark.parametrize("combo", ["PPN", "NND", "DDN", "NNN", "PDD"])
+@pytest.mark.parametrize("combo", ["PPN", "NND", "DDN", "NNN", "PDD", "PPP", "NDP", "DDP"])
 def test_partition_matches_oracle(nz, combo):
     """Plane of 8 x 20-ish systems: ragged last CTA (the plane is not a multiple of 32 systems)."""
     bc = wl.parse_bc(combo)
@@ -30,7 +30,7 @@ def test_partition_matches_oracle(nz, combo):
         assert e <= TOL, (alg, nz, combo, e)
 
 
-@pytest.mark.parametrize("combo", ["PPN", "NNN", "DDD", "NDN"])
+@pytest.mark.parametrize("combo", ["PPN", "NNN", "DDD", "NDN", "PPP", "NNP"])
 def test_partition_small_shift_modes(combo):
     """Strongly anisotropic spacing (dz << dx): |s| = dz^2 (lam_x/dx^2 + lam_y/dy^2) is tiny for the
     low modes, the pivots stay near -1 and the interface system is at its worst conditioned."""
@@ -48,7 +48,7 @@ def test_partition_large_shift_modes():
     """dz >> dx: |b| is large, the leading minors grow like |b|^R (no overflow, no loss of accuracy)."""
     shape = (128, 32, 32)
     h = (1.0 / 2048, 1.0 / 2048, 1.0 / 16)
-    for combo in ("PPN", "DDD"):
+    for combo in ("PPN", "DDD", "PPP"):
         bc = wl.parse_bc(combo)
         f = wl.random_normal(shape, 78, zero_mean=all(b in (0, 1) for b in bc))
         ref = po.solve(f, h, bc)
@@ -58,7 +58,7 @@ def test_partition_large_shift_modes():
 
 def test_partition_refused_where_it_does_not_apply():
     import paper_1909_05423_b200 as pp
-    for nz, combo in ((48, "PPN"), (256, "PPP"), (100, "DDD")):
+    for nz, combo in ((48, "PPN"), (768, "PPP"), (100, "DDD")):
         plan = pp.Plan(8, 8, nz, 0.1, 0.1, 0.1, combo)
         with pytest.raises(pp.PittPackError):
             plan.set_z_algorithm("partition")
