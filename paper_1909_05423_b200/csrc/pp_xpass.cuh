@@ -204,27 +204,32 @@ __device__ __forceinline__ void xinv_tile(const double *in, double *out, long lo
         // need the same two coefficients, and conj(w_{N-m}) = i w_m.  The owner of m in [0, N/2) loads the
         // pair once, keeps V_m and hands V_{N-m} to its owner through shared memory, exactly as above.
         // Packed rows: Y = Ya + i Yb, so Y_m - i Y_{N-m} = (ya + ybp) + i (yb - yap).
+        // (all loads first, so that they are in flight together; then the arithmetic)
+        double la[E / 2], lb[E / 2], lap[E / 2], lbp[E / 2], ha = 0.0, hb = 0.0;
 #pragma unroll
         for (int q = 0; q < E / 2; ++q) {
             const int m = t + q * P;
-            double ya, yb, yap = 0.0, ybp = 0.0;
-            if (bc == BC_N) {
-                ya = xld<LDCG>(ra + m); yb = xld<LDCG>(rb + m);
-                if (m > 0) { yap = xld<LDCG>(ra + N - m); ybp = xld<LDCG>(rb + N - m); }
-            } else {                                                   // Y'_m = (-1)^m S_{N-1-m}
-                const double s1 = sgn_of(m);
-                ya = s1 * xld<LDCG>(ra + N - 1 - m); yb = s1 * xld<LDCG>(rb + N - 1 - m);
-                if (m > 0) { yap = s1 * xld<LDCG>(ra + m - 1); ybp = s1 * xld<LDCG>(rb + m - 1); }   // (-1)^(N-m) S_{m-1}
+            const int at = (bc == BC_N) ? m : N - 1 - m, atp = (bc == BC_N) ? N - m : m - 1;
+            la[q] = xld<LDCG>(ra + at); lb[q] = xld<LDCG>(rb + at);
+            lap[q] = (m > 0) ? xld<LDCG>(ra + atp) : 0.0;
+            lbp[q] = (m > 0) ? xld<LDCG>(rb + atp) : 0.0;
+            if (m == 0) {                                              // thread 0 also makes V_{N/2} (its own partner)
+                const int ah = (bc == BC_N) ? H : N - 1 - H;
+                ha = xld<LDCG>(ra + ah); hb = xld<LDCG>(rb + ah);
             }
+        }
+#pragma unroll
+        for (int q = 0; q < E / 2; ++q) {
+            const int m = t + q * P;
+            const double s1 = (bc == BC_N) ? 1.0 : sgn_of(m);           // Dirichlet: Y'_m = (-1)^m S_{N-1-m}
+            const double ya = s1 * la[q], yb = s1 * lb[q], yap = s1 * lap[q], ybp = s1 * lbp[q];
             const double2 w = __ldg(&ptw[m]);
             v[q] = cmul(cconj(w), make_double2(ya + ybp, yb - yap));
             if (m > 0) {
-                s[lay(N - m)] = cmul(make_double2(w.y * -1.0, w.x), make_double2(yap + yb, ybp - ya));   // i w_m (...)
-            } else {                                                   // thread 0 also makes V_{N/2} (its own partner)
-                double ha, hb;
-                if (bc == BC_N) { ha = xld<LDCG>(ra + H); hb = xld<LDCG>(rb + H); }
-                else { const double sh = sgn_of(H); ha = sh * xld<LDCG>(ra + N - 1 - H); hb = sh * xld<LDCG>(rb + N - 1 - H); }
-                s[lay(H)] = cmul(cconj(__ldg(&ptw[H])), make_double2(ha + hb, hb - ha));
+                s[lay(N - m)] = cmul(make_double2(-w.y, w.x), make_double2(yap + yb, ybp - ya));   // i w_m (...)
+            } else {
+                const double sh = (bc == BC_N) ? 1.0 : sgn_of(H);
+                s[lay(H)] = cmul(cconj(__ldg(&ptw[H])), make_double2(sh * (ha + hb), sh * (hb - ha)));
             }
         }
     }

@@ -181,38 +181,48 @@ __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int compl
         // m in [0, N/2) loads the two rows once, keeps V_m and hands V_{N-m} to its owner through shared
         // memory (thread 0 also makes V_{N/2}).  A complex column inside such a tile (periodic x and y,
         // first tile) just loads its eight rows and takes part in the barriers.
+        // All loads first, so that they are in flight together; then the arithmetic.
+        // (the upper half of v is the landing place of the second row of each pair)
+        double2 yh = make_double2(0.0, 0.0);
 #pragma unroll
         for (int q = 0; q < E / 2; ++q) {
             const int m = t + q * P;                       // 0 <= m < N/2
             if (cplx) {
                 v[q] = base[m * ld];
                 v[q + E / 2] = base[(m + H) * ld];
-            } else if (bc == BC_P) {
-                if (m == 0) {                              // (A, B) both real: Z = A + i B
-                    v[q] = base[0];
-                    smem[lay(H)] = base[H * ld];
-                } else {
-                    const double2 lo = base[m * ld], hi = base[(N - m) * ld];
-                    v[q] = make_double2(lo.x - hi.y, hi.x + lo.y);
-                    smem[lay(N - m)] = make_double2(lo.x + hi.y, lo.y - hi.x);
-                }
+            } else if (bc == BC_P || bc == BC_N) {
+                v[q] = base[m * ld];
+                v[q + E / 2] = (m > 0) ? base[(N - m) * ld] : make_double2(0.0, 0.0);
+                if (m == 0) yh = base[H * ld];
             } else {
-                double2 ym, yp = make_double2(0.0, 0.0);
-                if (bc == BC_N) {
-                    ym = base[m * ld];
-                    if (m > 0) yp = base[(N - m) * ld];
+                v[q] = base[(N - 1 - m) * ld];
+                v[q + E / 2] = (m > 0) ? base[(m - 1) * ld] : make_double2(0.0, 0.0);
+                if (m == 0) yh = base[(N - 1 - H) * ld];
+            }
+        }
+        if (!cplx) {
+#pragma unroll
+            for (int q = 0; q < E / 2; ++q) {
+                const int m = t + q * P;
+                if (bc == BC_P) {
+                    if (m == 0) {                          // (A, B) both real: Z = A + i B
+                        smem[lay(H)] = yh;
+                    } else {
+                        const double2 lo = v[q], hi = v[q + E / 2];
+                        v[q] = make_double2(lo.x - hi.y, hi.x + lo.y);
+                        smem[lay(N - m)] = make_double2(lo.x + hi.y, lo.y - hi.x);
+                    }
                 } else {
-                    const double s1 = sgn_of(m);
-                    ym = dscale(s1, base[(N - 1 - m) * ld]);
-                    if (m > 0) yp = dscale(s1, base[(m - 1) * ld]);
-                }
-                const double2 wm = __ldg(&ptw[m]);
-                v[q] = cmul(cconj(wm), make_double2(ym.x + yp.y, ym.y - yp.x));
-                if (m > 0) {                               // conj(w_{N-m}) = i w_m
-                    smem[lay(N - m)] = cmul(make_double2(-wm.y, wm.x), make_double2(yp.x + ym.y, yp.y - ym.x));
-                } else {
-                    const double2 yh = (bc == BC_N) ? base[H * ld] : dscale(sgn_of(H), base[(N - 1 - H) * ld]);
-                    smem[lay(H)] = cmul(cconj(__ldg(&ptw[H])), make_double2(yh.x + yh.y, yh.y - yh.x));
+                    const double s1 = (bc == BC_N) ? 1.0 : sgn_of(m);  // Dirichlet: Y'_m = (-1)^m S_{N-1-m}
+                    const double2 a = dscale(s1, v[q]), b = dscale(s1, v[q + E / 2]);
+                    const double2 wm = __ldg(&ptw[m]);
+                    v[q] = cmul(cconj(wm), make_double2(a.x + b.y, a.y - b.x));
+                    if (m > 0) {                           // conj(w_{N-m}) = i w_m
+                        smem[lay(N - m)] = cmul(make_double2(-wm.y, wm.x), make_double2(b.x + a.y, b.y - a.x));
+                    } else {
+                        const double2 h2 = dscale((bc == BC_N) ? 1.0 : sgn_of(H), yh);
+                        smem[lay(H)] = cmul(cconj(__ldg(&ptw[H])), make_double2(h2.x + h2.y, h2.y - h2.x));
+                    }
                 }
             }
         }
