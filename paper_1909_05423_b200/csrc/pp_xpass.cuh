@@ -275,7 +275,9 @@ __global__ void __launch_bounds__(XCfg<N>::THREADS, PP_X_MINB)
 xpass_inv_kernel(const double *in, double *out, long long npairs, int bc,
                  const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
     extern __shared__ double2 smem[];
-    xinv_tile<N, XCfg<N>::T, false>(in, out, (long long)blockIdx.x * XCfg<N>::T, npairs, bc, tw, ptw, smem);
+    // rows from the last to the first: the y pass before this one went plane 0 to plane nz-1, so its
+    // last planes are still in L2
+    xinv_tile<N, XCfg<N>::T, false>(in, out, (long long)(gridDim.x - 1 - blockIdx.x) * XCfg<N>::T, npairs, bc, tw, ptw, smem);
 }
 
 }  // namespace pp

@@ -153,7 +153,9 @@ __global__ void __launch_bounds__(YCfg<N>::THREADS, YCfg<N>::MINB)
 ypass_fwd_kernel(double2 *w, int nxh, int bc, int complex_cols,
                  const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
     extern __shared__ double2 smem[];
-    yfwd_tile<N, false>(w, nxh, bc, complex_cols, tw, ptw, blockIdx.x, blockIdx.y, smem);
+    // planes from the last to the first: the x pass before this one went first to last, so the planes
+    // it wrote last are still (dirty) in L2 -- they are read from there and overwritten there
+    yfwd_tile<N, false>(w, nxh, bc, complex_cols, tw, ptw, blockIdx.x, gridDim.y - 1 - blockIdx.y, smem);
 }
 
 // One CTA-wide tile of the inverse y pass (see yfwd_tile).
