@@ -107,3 +107,40 @@ def test_error_codes_on_device():
     assert pp.pp_plan_destroy(h) == 0
     assert pp.pp_plan_destroy(0) == 0
     del n
+
+
+@pytest.mark.parametrize("case", ["cfg1", "fused128", "long768"])
+def test_pp_solve_is_graph_capturable(case):
+    """pp_solve never allocates and never synchronises (include/pittpack_b200.h), so a solve can be
+    captured into a CUDA graph and replayed -- what a time-stepping caller does with small grids,
+    where five launches cost more than the kernels (config 1: launch-latency bound)."""
+    import torch
+    import paper_1909_05423_b200 as pp
+    if case == "cfg1":
+        w = wl.config1("uniform")
+    elif case == "fused128":
+        w = wl.config2("PPN", "normal")
+    else:
+        shape = (768, 8, 16)
+        w = wl.Workload("long768", shape, (1.0 / 16, 1.0 / 8, 1.0 / 8), wl.parse_bc("NND"), wl.random_uniform(shape, 3))
+    nz, ny, nx = w.shape
+    plan = pp.Plan(nx, ny, nz, *w.h, w.bc)
+    if case == "fused128":
+        plan.set_xy_fusion(True)
+    f = torch.from_numpy(w.f).cuda()
+    u = torch.empty_like(f)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        plan.solve(f, u)                            # warm-up outside capture (function attributes, lazy module load)
+    s.synchronize()
+    ref = u.clone()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        plan.solve(f, u)
+    u.zero_()
+    g.replay()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(u, ref)
+    assert rel_err(u.cpu().numpy(), po.solve(w.f, w.h, w.bc)) <= TOL
+    plan.destroy()
