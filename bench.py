@@ -44,6 +44,8 @@ def workload_by_name(name):
         return wl.config1("uniform")
     if name == "pencil":
         return wl.paper_pencil("PPN")
+    if name == "pencil48":
+        return wl.paper_pencil("PPN", nxy=48, nz=8192)
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -355,7 +357,7 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="cfg3", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "pencil"])
+    ap.add_argument("--workload", default="cfg3", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "pencil", "pencil48"])
     ap.add_argument("--fusion", action="store_true", help="plane-wise x+y fusion through L2 (opt-in, DESIGN.md)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

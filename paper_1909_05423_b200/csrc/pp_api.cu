@@ -49,15 +49,17 @@ namespace {
 
 const long double PI_L = 3.14159265358979323846264338327950288L;
 
-bool pow2_in_range(int n) { return n >= 4 && n <= 2048 && (n & (n - 1)) == 0; }
+// powers of two in [4, 2048], 3 * 2^k in [48, 1536], 5 * 2^k in [80, 1280]
+bool length_supported(int n) { return n >= 4 && n <= 2048 && fft_length_ok(n); }
 
 void make_twiddles(int n, std::vector<double2> &tw, std::vector<double2> &ptw) {
     tw.assign(tw_table_elems(n), make_double2(1.0, 0.0));
     ptw.resize(n + 1);
-    // stage with NS (radix 8): rows r = 1, 2, 4 of W_n^(k r stride), stride = n / (8 NS), k in [0, NS)
-    for (int ns = first_radix(n); ns < n; ns *= 8) {
-        const int off = tw_stage_offset(n, ns), stride = n / (8 * ns);
-        for (int ri = 0; ri < 3; ++ri)
+    // stage with NS: rows r = 1, 2, 4 (radix 8) or r = 1, 2 (radix 4) of W_n^(k r stride), stride = n / (RS NS), k in [0, NS)
+    const int rs = stage_radix(n), rows = tw_rows(n);
+    for (int ns = first_radix(n); ns < n; ns *= rs) {
+        const int off = tw_stage_offset(n, ns), stride = n / (rs * ns);
+        for (int ri = 0; ri < rows; ++ri)
             for (int k = 0; k < ns; ++k) {
                 const long long e = ((long long)k * (1 << ri) * stride) % n;
                 const long double a = 2.0L * PI_L * (long double)e / (long double)n;
@@ -152,6 +154,17 @@ int launch_y(bool fwd, double *w, int nxh, int nz, int bc, int complex_cols, con
         case 512:  return CALL(512);                 \
         case 1024: return CALL(1024);                \
         case 2048: return CALL(2048);                \
+        case 48:   return CALL(48);                  \
+        case 96:   return CALL(96);                  \
+        case 192:  return CALL(192);                 \
+        case 384:  return CALL(384);                 \
+        case 768:  return CALL(768);                 \
+        case 1536: return CALL(1536);                \
+        case 80:   return CALL(80);                  \
+        case 160:  return CALL(160);                 \
+        case 320:  return CALL(320);                 \
+        case 640:  return CALL(640);                 \
+        case 1280: return CALL(1280);                \
         default:   return PP_ERR_UNSUPPORTED_SIZE;   \
     }
 
@@ -317,7 +330,7 @@ const char *pp_strerror(int status) {
     switch (status) {
         case PP_SUCCESS: return "success";
         case PP_ERR_INVALID_ARG: return "invalid argument";
-        case PP_ERR_UNSUPPORTED_SIZE: return "unsupported grid size (nx, ny: powers of two in [4, 2048]; nz in [2, 4096], or 256 m <= 16384 with non-periodic z)";
+        case PP_ERR_UNSUPPORTED_SIZE: return "unsupported grid size (nx, ny: 2^k in [4, 2048], 3*2^k in [48, 1536] or 5*2^k in [80, 1280]; nz in [2, 4096], or 256 m <= 16384 with non-periodic z)";
         case PP_ERR_ALLOC: return "allocation failed";
         case PP_ERR_CUDA: return "CUDA runtime or launch error (is a CUDA device present?)";
         case PP_ERR_NULL: return "null pointer argument";
@@ -337,7 +350,7 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
     // nz: the two-sweep kernels take any nz up to 4096; longer lines need the two-level partition
     // (Neumann / Dirichlet z, nz a multiple of 256 up to 16384)
     const bool long_ok = bc_z != PP_BC_PERIODIC && zpart_hier_ok(nz);
-    if (!pow2_in_range(nx) || !pow2_in_range(ny) || nz < 2 || (nz > 64 * Z_MAX_CK && !long_ok)) return PP_ERR_UNSUPPORTED_SIZE;
+    if (!length_supported(nx) || !length_supported(ny) || nz < 2 || (nz > 64 * Z_MAX_CK && !long_ok)) return PP_ERR_UNSUPPORTED_SIZE;
 
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }

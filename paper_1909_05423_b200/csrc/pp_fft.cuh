@@ -1,17 +1,19 @@
 // Complex FFT core shared by the x- and y-pass kernels: a register + shared-memory Stockham
-// autosort FFT, radix 8 (leading radix 2 or 4 when log2 N is not a multiple of 3), fp64.
+// autosort FFT, fp64.  Powers of two: radix 8 (leading radix 2 or 4 when log2 N is not a multiple
+// of 3).  3 * 2^k and 5 * 2^k: a leading prime-factor butterfly of 6 / 12 / 10 / 20 points, then radix 4.
 //
 // "PittPack performs complex FFT transform for all the transformations": every
 // periodic / Neumann / Dirichlet transform of the solver is this core plus a fused pre- and
 // post-processing step.  The paper calls cuFFT here; this is the hand-written
 // replacement.
 //
-// Thread mapping.  An N-point transform is done by P = N/E threads, E = min(8, N) elements per
-// thread.  Thread t holds, before and after every stage and on exit, the elements with index
-// t + m*P (m = 0..E-1) in natural order -- so global loads and stores of consecutive threads are
-// contiguous, and the last stage needs no shared-memory round trip.  Between stages the data is
-// exchanged through shared memory (one store + one load of each element), padded by one element
-// every eight so that every 16-byte access pattern of the schedule is bank-conflict free.
+// Thread mapping.  An N-point transform is done by P = N/E threads, E elements per thread (8 for
+// powers of two, 12 or 20 otherwise).  Thread t holds, before and after every stage and on exit, the
+// elements with index t + m*P (m = 0..E-1) in natural order -- so global loads and stores of
+// consecutive threads are contiguous, and the last stage needs no shared-memory round trip.  A stage
+// of radix R does E/R butterflies per thread.  Between stages the data is exchanged through shared
+// memory (one store + one load of each element), padded by one element every eight so that every
+// 16-byte access pattern of the power-of-two schedule is bank-conflict free.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -22,30 +24,53 @@ constexpr int INV = +1;   // exp(+2 pi i k n / N), unnormalised
 
 __host__ __device__ constexpr int ilog2(int n) { return n <= 1 ? 0 : 1 + ilog2(n >> 1); }
 
+// Supported lengths: N = odd * 2^k with odd in {1, 3, 5} -- the powers of two of BASELINE.json's grids
+// and the 48- and 80-multiples of the paper's weak-scaling runs.
+//   odd = 1: E = 8 elements per thread, radix-8 stages after a first stage of radix 2, 4 or 8
+//   odd = 3: E = 12, radix-4 stages after a first stage of radix 12 (k even) or 6 (k odd)
+//   odd = 5: E = 20, radix-4 stages after a first stage of radix 20 (k even) or 10 (k odd)
+// The first stage has no twiddles; its composite butterflies (6, 10, 12, 20) are prime-factor
+// (Good-Thomas) combinations of a 3- or 5-point and a 2- or 4-point DFT, so they need none inside either.
+__host__ __device__ constexpr int fft_odd_part(int n) { return (n % 2 == 0) ? fft_odd_part(n / 2) : n; }
+__host__ __device__ constexpr int fft_log2_part(int n) { return ilog2(n / fft_odd_part(n)); }
+__host__ __device__ constexpr bool fft_length_ok(int n) {
+    return n >= 4 && (fft_odd_part(n) == 1 || ((fft_odd_part(n) == 3 || fft_odd_part(n) == 5) && fft_log2_part(n) >= 4));
+}
+__host__ __device__ constexpr int stage_radix(int n) { return fft_odd_part(n) == 1 ? 8 : 4; }   // every stage after the first
+__host__ __device__ constexpr int first_radix(int n) {
+    return fft_odd_part(n) == 1 ? ((ilog2(n) % 3 == 0) ? 8 : ((ilog2(n) % 3 == 1) ? 2 : 4))
+                                : fft_odd_part(n) * ((fft_log2_part(n) % 2 == 0) ? 4 : 2);
+}
+
 template <int N>
 struct FftCfg {
-    static_assert(N >= 4 && (N & (N - 1)) == 0, "power of two >= 4");
-    static constexpr int LOG2 = ilog2(N);
-    static constexpr int E = N >= 8 ? 8 : N;       // elements per thread
+    static_assert(fft_length_ok(N), "N = 2^k >= 4, or 3 * 2^k / 5 * 2^k with k >= 4");
+    static constexpr int ODD = fft_odd_part(N);
+    static constexpr int E = (ODD == 1) ? (N >= 8 ? 8 : N) : 4 * ODD;   // elements per thread
     static constexpr int P = N / E;                // threads per transform
-    static constexpr int R0 = (LOG2 % 3 == 0) ? 8 : ((LOG2 % 3 == 1) ? 2 : 4);   // first radix
+    static constexpr int RS = stage_radix(N);      // radix of every stage after the first
+    static constexpr int R0 = first_radix(N);      // first radix
     static constexpr int SMEM_ELEMS = N + N / 8;   // double2 elements per transform incl. padding
 };
 
-// Stage twiddle tables.  Every stage after the first is radix 8 and multiplies input r of butterfly
-// j by W_N^(k r STRIDE), k = j mod NS, STRIDE = N / (8 NS).  The plan stores, per stage, the three
-// rows r = 1, 2, 4 as [r][k] -- contiguous in k, so a warp's 16-byte loads touch NS*16 contiguous
-// bytes (one L1 line for NS = 8, four for NS >= 32) instead of lines STRIDE*16 bytes apart; the other
-// powers are products.  Stage with NS starts at element 3 * (sum of the earlier stages' NS).
-__host__ __device__ constexpr int first_radix(int n) {
-    return (ilog2(n) % 3 == 0) ? 8 : ((ilog2(n) % 3 == 1) ? 2 : 4);
-}
+// Stage twiddle tables.  Every stage after the first has radix RS (8 or 4) and multiplies input r of
+// butterfly j by W_N^(k r STRIDE), k = j mod NS, STRIDE = N / (RS NS).  The plan stores, per stage, the
+// rows r = 1, 2, 4 (RS = 8) or r = 1, 2 (RS = 4) as [r][k] -- contiguous in k, so a warp's 16-byte loads
+// touch NS*16 contiguous bytes instead of lines STRIDE*16 bytes apart; the other powers are products.
+__host__ __device__ constexpr int tw_rows(int n) { return stage_radix(n) == 8 ? 3 : 2; }
 __host__ __device__ constexpr int tw_stage_offset(int n, int NS) {
     int off = 0;
-    for (int ns = first_radix(n); ns < NS; ns *= 8) off += 3 * ns;
+    for (int ns = first_radix(n); ns < NS; ns *= stage_radix(n)) off += tw_rows(n) * ns;
     return off;
 }
 __host__ __device__ constexpr int tw_table_elems(int n) { return tw_stage_offset(n, n) > 0 ? tw_stage_offset(n, n) : 1; }
+
+// (N - m) mod N for 0 <= m < N
+template <int N>
+__device__ __forceinline__ int neg_mod(int m) {
+    if constexpr ((N & (N - 1)) == 0) return (N - m) & (N - 1);
+    else return m == 0 ? 0 : N - m;
+}
 
 __device__ __forceinline__ int pad8(int i) { return i + (i >> 3); }
 
@@ -102,11 +127,80 @@ __device__ __forceinline__ void bfly8(double2 (&x)[8]) {
     x[3] = cadd(e3, o3); x[7] = csub(e3, o3);
 }
 
+// in-place natural-order 3-point DFT
+template <int DIR>
+__device__ __forceinline__ void bfly3(double2 &x0, double2 &x1, double2 &x2) {
+    constexpr double S = 0.86602540378443864676;   // sin(2 pi / 3)
+    const double2 t = cadd(x1, x2), u = csub(x1, x2);
+    const double2 m = make_double2(fma(-0.5, t.x, x0.x), fma(-0.5, t.y, x0.y));
+    // forward: x1' = m - i S u, x2' = m + i S u;  inverse: the other way round
+    const double2 r = DIR == FWD ? make_double2(S * u.y, -S * u.x) : make_double2(-S * u.y, S * u.x);
+    x0 = cadd(x0, t);
+    x1 = cadd(m, r);
+    x2 = csub(m, r);
+}
+
+// in-place natural-order 5-point DFT
+template <int DIR>
+__device__ __forceinline__ void bfly5(double2 &x0, double2 &x1, double2 &x2, double2 &x3, double2 &x4) {
+    constexpr double C1 = 0.30901699437494742410, C2 = -0.80901699437494742410;   // cos(2 pi/5), cos(4 pi/5)
+    constexpr double S1 = 0.95105651629515357212, S2 = 0.58778525229247312917;    // sin(2 pi/5), sin(4 pi/5)
+    const double2 a = cadd(x1, x4), b = csub(x1, x4), c = cadd(x2, x3), d = csub(x2, x3);
+    const double2 m1 = make_double2(x0.x + C1 * a.x + C2 * c.x, x0.y + C1 * a.y + C2 * c.y);
+    const double2 m2 = make_double2(x0.x + C2 * a.x + C1 * c.x, x0.y + C2 * a.y + C1 * c.y);
+    const double2 n1 = make_double2(S1 * b.x + S2 * d.x, S1 * b.y + S2 * d.y);
+    const double2 n2 = make_double2(S2 * b.x - S1 * d.x, S2 * b.y - S1 * d.y);
+    // forward: X_k = m -/+ i n  (k = 1, 2 take "- i n"), inverse: conjugate pattern
+    const double2 r1 = DIR == FWD ? make_double2(n1.y, -n1.x) : make_double2(-n1.y, n1.x);
+    const double2 r2 = DIR == FWD ? make_double2(n2.y, -n2.x) : make_double2(-n2.y, n2.x);
+    x0 = cadd(x0, cadd(a, c));
+    x1 = cadd(m1, r1);
+    x4 = csub(m1, r1);
+    x2 = cadd(m2, r2);
+    x3 = csub(m2, r2);
+}
+
+// in-place natural-order DFT of length R = A * B, A in {3, 5}, B in {2, 4}: prime-factor (Good-Thomas)
+// algorithm.  With input n = (B n1 + A n2) mod R and output k = (B b' k1 + A a' k2) mod R, where
+// b' = B^-1 mod A and a' = A^-1 mod B, the kernel factors exactly into W_A^(n1 k1) W_B^(n2 k2): A-point
+// DFTs over n1, then B-point DFTs over n2, no twiddles in between.  All index maps are compile-time.
+__host__ __device__ constexpr int inv_mod(int a, int m) {
+    for (int i = 1; i < m; ++i) if ((a * i) % m == 1) return i;
+    return 1;
+}
+template <int A, int B, int DIR>
+__device__ __forceinline__ void bfly_pfa(double2 (&x)[A * B]) {
+    constexpr int R = A * B;
+    double2 y[A][B];
+#pragma unroll
+    for (int n2 = 0; n2 < B; ++n2) {
+        double2 c[A];
+#pragma unroll
+        for (int n1 = 0; n1 < A; ++n1) c[n1] = x[(B * n1 + A * n2) % R];
+        if constexpr (A == 3) bfly3<DIR>(c[0], c[1], c[2]);
+        else bfly5<DIR>(c[0], c[1], c[2], c[3], c[4]);
+#pragma unroll
+        for (int k1 = 0; k1 < A; ++k1) y[k1][n2] = c[k1];
+    }
+    constexpr int CB = B * inv_mod(B % A, A), CA = A * inv_mod(A % B, B);
+#pragma unroll
+    for (int k1 = 0; k1 < A; ++k1) {
+        if constexpr (B == 2) bfly2<DIR>(y[k1][0], y[k1][1]);
+        else bfly4<DIR>(y[k1][0], y[k1][1], y[k1][2], y[k1][3]);
+#pragma unroll
+        for (int k2 = 0; k2 < B; ++k2) x[(CB * k1 + CA * k2) % R] = y[k1][k2];
+    }
+}
+
 template <int R, int DIR>
 __device__ __forceinline__ void bfly(double2 (&x)[R]) {
     if constexpr (R == 2) bfly2<DIR>(x[0], x[1]);
     else if constexpr (R == 4) bfly4<DIR>(x[0], x[1], x[2], x[3]);
-    else bfly8<DIR>(x);
+    else if constexpr (R == 8) bfly8<DIR>(x);
+    else if constexpr (R == 6) bfly_pfa<3, 2, DIR>(x);
+    else if constexpr (R == 12) bfly_pfa<3, 4, DIR>(x);
+    else if constexpr (R == 10) bfly_pfa<5, 2, DIR>(x);
+    else bfly_pfa<5, 4, DIR>(x);
 }
 
 // One Stockham stage of radix R with NS = product of the previous radices.
@@ -126,9 +220,8 @@ __device__ __forceinline__ void fft_stage(double2 (&v)[FftCfg<N>::E], int t, dou
         double2 x[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) x[r] = v[b + B * r];
-        const int k = j & (NS - 1);
-        if constexpr (NS > 1) {
-            static_assert(R == 8, "every stage after the first is radix 8");
+        const int k = j % NS;
+        if constexpr (NS > 1 && R == 8) {
             // W^(k r STRIDE): load r = 1, 2, 4 from the stage table, build the rest with one product each
             const double2 *ts = tw + tw_stage_offset(N, NS);
             double2 w1 = __ldg(&ts[k]);
@@ -143,6 +236,15 @@ __device__ __forceinline__ void fft_stage(double2 (&v)[FftCfg<N>::E], int t, dou
             x[5] = cmul(x[5], cmul(w1, w4));
             x[6] = cmul(x[6], cmul(w2, w4));
             x[7] = cmul(x[7], cmul(w3, w4));
+        } else if constexpr (NS > 1) {
+            static_assert(R == 4, "stages after the first are radix 8 (powers of two) or radix 4 (3 * 2^k, 5 * 2^k)");
+            const double2 *ts = tw + tw_stage_offset(N, NS);
+            double2 w1 = __ldg(&ts[k]);
+            double2 w2 = __ldg(&ts[NS + k]);
+            if (DIR == INV) { w1 = cconj(w1); w2 = cconj(w2); }
+            x[1] = cmul(x[1], w1);
+            x[2] = cmul(x[2], w2);
+            x[3] = cmul(x[3], cmul(w1, w2));
         }
         bfly<R, DIR>(x);
         if constexpr (LAST) {
@@ -165,7 +267,7 @@ __device__ __forceinline__ void fft_stage(double2 (&v)[FftCfg<N>::E], int t, dou
 template <int N, int NS, int DIR, class Layout, class Sync>
 __device__ __forceinline__ void fft_stages(double2 (&v)[FftCfg<N>::E], int t, double2 *s,
                                            const double2 *__restrict__ tw, const Layout &lay, const Sync &sync) {
-    constexpr int R = (NS == 1) ? FftCfg<N>::R0 : 8;
+    constexpr int R = (NS == 1) ? FftCfg<N>::R0 : FftCfg<N>::RS;
     fft_stage<N, R, NS, DIR>(v, t, s, tw, lay, sync);
     if constexpr (NS * R < N) fft_stages<N, NS * R, DIR>(v, t, s, tw, lay, sync);
 }

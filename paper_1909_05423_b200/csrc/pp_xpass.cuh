@@ -51,6 +51,7 @@ struct XCfg {
     static constexpr int P = FftCfg<N>::P;
     static constexpr int T = (256 / P) > 0 ? (256 / P) : 1;   // transforms (row pairs) per CTA; <= 4 when P >= 64
     static constexpr int THREADS = T * P;
+    static constexpr int MINB = (FftCfg<N>::E <= 12) ? PP_X_MINB : 2;   // 20 elements per thread need more than 64 registers
     static constexpr size_t SMEM = size_t(T) * FftCfg<N>::SMEM_ELEMS * sizeof(double2);
 };
 
@@ -104,7 +105,7 @@ __device__ __forceinline__ void xfwd_tile(const double *in, double *out, long lo
         for (int q = 0; q < E / 2; ++q) {
             const int m = t + q * P;                       // 0 <= m < N/2
             const double2 zm = v[q];
-            const double2 zc = s[lay((N - m) & (N - 1))];
+            const double2 zc = s[lay(neg_mod<N>(m))];
             if (m == 0) {
                 const double2 zh = v[E / 2];               // thread 0 also holds Z_{N/2}
                 if (bc == BC_P) {
@@ -147,7 +148,7 @@ __device__ __forceinline__ void xfwd_tile(const double *in, double *out, long lo
 
 
 template <int N>
-__global__ void __launch_bounds__(XCfg<N>::THREADS, PP_X_MINB)
+__global__ void __launch_bounds__(XCfg<N>::THREADS, XCfg<N>::MINB)
 xpass_fwd_kernel(const double *in, double *out, long long npairs, int bc,
                  const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
     extern __shared__ double2 smem[];
@@ -271,7 +272,7 @@ __device__ __forceinline__ void xinv_tile(const double *in, double *out, long lo
 }
 
 template <int N>
-__global__ void __launch_bounds__(XCfg<N>::THREADS, PP_X_MINB)
+__global__ void __launch_bounds__(XCfg<N>::THREADS, XCfg<N>::MINB)
 xpass_inv_kernel(const double *in, double *out, long long npairs, int bc,
                  const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
     extern __shared__ double2 smem[];

@@ -109,7 +109,7 @@ __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int compl
     for (int q = 0; q < E / 2; ++q) {
         const int m = t + q * P;
         const double2 zm = v[q];
-        const double2 zc = smem[lay((N - m) & (N - 1))];
+        const double2 zc = smem[lay(neg_mod<N>(m))];
         if (m == 0) {
             const double2 zh = v[E / 2];
             if (bc == BC_P) {

@@ -143,9 +143,10 @@ def config3(scale: int = 1) -> Workload:
 
 
 def paper_pencil(combo: str = "PPN", nxy: int = 64, nz: int = 16384) -> Workload:
-    """The paper's own per-GPU weak-scaling load: a 64 x 64 x 16384 pencil (Fig. 8
-    caption), cubic cells h = 1/nxy (domain 1 x 1 x nz/nxy); N(0,1), projected to zero
-    mean when the problem is singular.  Only 4096 tridiagonal systems, each 16384 long."""
+    """The paper's own per-GPU weak-scaling loads: a 64 x 64 x 16384 pencil (Fig. 8
+    caption, PAPER.md:332) or, with nxy = 48 and nz = 8192, the 48 x 48 x 8192 one (PAPER.md:611);
+    cubic cells h = 1/nxy (domain 1 x 1 x nz/nxy); N(0,1), projected to zero mean when the problem is
+    singular.  Only nxy^2 tridiagonal systems, each nz long."""
     shape, h, bc = (nz, nxy, nxy), (1.0 / nxy,) * 3, parse_bc(combo)
     f = random_normal(shape, seed_for(6, 0), zero_mean=all(b in (P, N) for b in bc))
     return Workload(f"pencil-{nxy}x{nxy}x{nz}-{combo}-normal", shape, h, bc, f)

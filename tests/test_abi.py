@@ -49,7 +49,9 @@ def test_validation_without_device():
     assert pp.pp_plan_create(32, 32, 32, -0.1, 0.1, 0.1, 0, 0, 0)[0] == 1     # non-positive spacing
     assert pp.pp_plan_create(32, 32, 32, 0.1, 0.1, float("nan"), 0, 0, 0)[0] == 1
     assert pp.pp_plan_create(32, 32, 32, 0.1, 0.1, 0.1, 0, 3, 0)[0] == 1      # unknown BC
-    assert pp.pp_plan_create(48, 32, 32, 0.1, 0.1, 0.1, 0, 0, 0)[0] == 2      # not a power of two
+    assert pp.pp_plan_create(36, 32, 32, 0.1, 0.1, 0.1, 0, 0, 0)[0] == 2      # not 2^k, 3*2^k (k >= 4) or 5*2^k (k >= 4)
+    assert pp.pp_plan_create(32, 24, 32, 0.1, 0.1, 0.1, 0, 0, 0)[0] == 2      # 3*2^3: too short for the mixed-radix schedule
+    assert pp.pp_plan_create(32, 112, 32, 0.1, 0.1, 0.1, 0, 0, 0)[0] == 2     # 7*2^4
     assert pp.pp_plan_create(32, 4096, 32, 0.1, 0.1, 0.1, 0, 0, 0)[0] == 2    # too long
     assert pp.pp_plan_create(32, 32, 1, 0.1, 0.1, 0.1, 0, 0, 0)[0] == 2       # nz < 2
     assert pp.pp_plan_destroy(0) == 0

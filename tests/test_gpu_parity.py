@@ -48,6 +48,32 @@ def test_every_fft_length(n, axis, bc_t):
     check(wl.Workload(f"len{n}{axis}{bc_t}", shape, h, wl.parse_bc(combo), f))
 
 
+@pytest.mark.parametrize("n", [48, 96, 192, 384, 768, 1536, 80, 160, 320, 640, 1280])
+@pytest.mark.parametrize("axis", ["x", "y"])
+@pytest.mark.parametrize("bc_t", "PND")
+def test_every_mixed_radix_length(n, axis, bc_t):
+    """3*2^k and 5*2^k lengths (the 48-multiples of the paper's weak-scaling grids):
+    prime-factor first stage + radix-4 stages, each transform type on each axis."""
+    other = 4 if n >= 512 else 8
+    nx, ny = (n, other) if axis == "x" else (other, n)
+    nz = 3
+    combo = (bc_t + "N" + "D") if axis == "x" else ("D" + bc_t + "N")
+    shape = (nz, ny, nx)
+    h = (1.0 / nx, 1.0 / ny, 0.5)
+    f = wl.random_uniform(shape, 3 * n + (0 if axis == "x" else 1))
+    check(wl.Workload(f"len{n}{axis}{bc_t}", shape, h, wl.parse_bc(combo), f))
+
+
+@pytest.mark.parametrize("combo", ALL27)
+def test_all_27_combos_on_a_48_multiple(combo):
+    """48 x 96 x 40: the paper's 48-multiple grid shape, every boundary-condition combination."""
+    bc = wl.parse_bc(combo)
+    shape = (40, 96, 48)
+    h = (1.0 / 48, 1.0 / 96, 1.0 / 40)
+    f = wl.random_normal(shape, 48 + ALL27.index(combo), zero_mean=all(b in (0, 1) for b in bc))
+    check(wl.Workload(f"mixed-{combo}", shape, h, bc, f))
+
+
 def test_config1_both_variants():
     for variant in ("mms", "uniform"):
         w = wl.config1(variant)

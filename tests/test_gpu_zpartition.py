@@ -99,6 +99,14 @@ def test_paper_pencil_shape(combo):
     print(f"pencil {combo}: gpu vs long-double oracle {e:.2e}; fp64 oracle vs long-double oracle {e64:.2e}")
 
 
+def test_paper_pencil_48():
+    """48 x 48 x 8192: mixed-radix transforms and the two-level z solve together."""
+    w = wl.paper_pencil("PPN", nxy=48, nz=8192)
+    ref = po.solve(w.f, w.h, w.bc, zdtype=np.longdouble)
+    e = rel_err(gpu_solve(w.f, w.h, w.bc), ref)
+    assert e <= TOL, e
+
+
 def test_long_line_limits():
     import paper_1909_05423_b200 as pp
     for nz, combo, ok in ((8192, "PPN", True), (8192, "PPP", False), (8192 + 128, "PPN", False), (32768, "PPD", False)):
