@@ -68,7 +68,7 @@ __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int compl
     const int cp = bx * T + c;
     const bool active = cp < nxh;
     double2 *base = w + (size_t)z * N * nxh + (active ? cp : 0);
-    const size_t ld = nxh;
+    const int ld = nxh;                                    // row offsets inside a plane fit 32 bits
     const LayoutCol<T> lay{c};
     const SyncCta sync;
 
@@ -169,7 +169,7 @@ __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int compl
     const int cp = bx * T + c;
     const bool active = cp < nxh;
     double2 *base = w + (size_t)z * N * nxh + (active ? cp : 0);
-    const size_t ld = nxh;
+    const int ld = nxh;                                    // row offsets inside a plane fit 32 bits
     const LayoutCol<T> lay{c};
     const SyncCta sync;
     const bool cplx = complex_cols && cp > 0;
