@@ -28,9 +28,13 @@
 // [j R, (j+1) R).  All R loads of a thread are issued before anything else, so a resident CTA has
 // its whole tile (L nz doubles) in flight.
 //
-// Neumann / Dirichlet z only (periodic z keeps the Sherman-Morrison kernel); nz must
-// be R S with R in {32, 64}; other sizes keep the two-sweep kernel.  The singular (0,0) line is
-// handled by zero_mode_line exactly as there.
+// Periodic z (template flag CYC): every segment is an interior block and the interface chain closes on
+// itself; the two wrap-around couplings are folded in by a 2x2 closure (see the kernel) -- an exact
+// cyclic solve in place of the Sherman-Morrison correction of PAPER.md:216.
+//
+// nz must be R S with R in {32, 64} (zpart_shape); longer Neumann / Dirichlet lines (nz = 256 m) use the
+// same kernel on two levels (ZHier, MODE 1 / 2); everything else keeps the two-sweep kernels of
+// pp_zsolve.cuh.  The singular (0,0) line is handled by zero_mode_line exactly as there.
 #pragma once
 #include "pp_zsolve.cuh"
 
@@ -161,8 +165,8 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
 #pragma unroll
     for (int i = 0; i < R; ++i) y[i] = __ldcs(row0 + i * step);
 
-    // While the loads fly: segment 0's thread tabulates the first block, segment 1's the interior
-    // block, segment 2's (segment 1's when S = 2) factors the interface matrix.
+    // While the loads fly: thread 0 of the system tabulates the first block, thread jint the interior
+    // block, thread jfac factors the interface matrix.
     if (j <= jfac) {
         const double bint = -2.0 + s;
         const double bend = ((p.bcz == 1) ? -1.0 : -3.0) + s;

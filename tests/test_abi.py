@@ -54,6 +54,12 @@ def test_validation_without_device():
     assert pp.pp_plan_create(32, 112, 32, 0.1, 0.1, 0.1, 0, 0, 0)[0] == 2     # 7*2^4
     assert pp.pp_plan_create(32, 4096, 32, 0.1, 0.1, 0.1, 0, 0, 0)[0] == 2    # too long
     assert pp.pp_plan_create(32, 32, 1, 0.1, 0.1, 0.1, 0, 0, 0)[0] == 2       # nz < 2
+    assert pp.pp_plan_create(32, 32, 8192, 0.1, 0.1, 0.1, 0, 0, 0)[0] == 2    # long lines need non-periodic z
+    assert pp.pp_plan_create(32, 32, 8192 + 64, 0.1, 0.1, 0.1, 0, 0, 1)[0] == 2   # ... and nz = 256 m
+    assert pp.pp_plan_create(32, 32, 32768, 0.1, 0.1, 0.1, 0, 0, 1)[0] == 2   # ... up to 16384
+    assert pp.binding.pp_plan_set_z_algorithm(0, 1) == 5                      # NULL plan
+    assert pp.binding.pp_plan_set_xy_fusion(0, 1) == 5
+    assert pp.binding.pp_plan_launches_per_solve(0) == 0
     assert pp.pp_plan_destroy(0) == 0
     assert pp.pp_solve(0, 0, 0) == 5
     assert pp.pp_plan_workspace_bytes(0) == 0
