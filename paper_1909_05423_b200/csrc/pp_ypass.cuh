@@ -20,6 +20,8 @@
 // In every case the modified wavenumber of row m is Table 2's evaluated at m,
 // because the periodic eigenvalue is even in m -- so the z solve needs one table per axis.
 #pragma once
+#include <type_traits>
+
 #include "pp_xpass.cuh"
 
 namespace pp {
@@ -28,6 +30,24 @@ template <int T>
 struct LayoutCol {
     int c;
     __device__ __forceinline__ int operator()(int i) const { return pad8(i) * T + c; }
+};
+
+// Tiles of 4 columns (N > 512): a quarter-warp -- the unit a 16-byte shared-memory access is served
+// in -- is 4 columns x 2 consecutive rows (t even, t + 1), so the two rows must land in different halves
+// of a 128-byte bank row.  The padded layout does that for the row patterns of radix-8 stages only; the
+// leading radix-2 / radix-4 stage of the 1024- and 2048-point transforms stores rows that differ by
+// R0 = 2^S and conflicts two-way.  Here the low bit of the row is XORed with bit S instead: rows i, i+1
+// (i even: every load, every later store) and rows i, i + R0 (the first stage's stores) then always differ
+// in that bit.  No padding needed.
+template <int S>
+struct LayoutColXor4 {
+    int c;
+    __device__ __forceinline__ int operator()(int i) const { return ((i ^ ((i >> S) & 1)) << 2) + c; }
+};
+template <int N, int T>
+struct YLayout {
+    static constexpr bool XOR4 = (T == 4) && ((N & (N - 1)) == 0) && (FftCfg<N>::R0 == 2 || FftCfg<N>::R0 == 4);
+    using type = typename std::conditional<XOR4, LayoutColXor4<FftCfg<N>::R0 == 2 ? 1 : 2>, LayoutCol<T>>::type;
 };
 
 struct SyncCta {
@@ -69,7 +89,7 @@ __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int compl
     const bool active = cp < nxh;
     double2 *base = w + (size_t)z * N * nxh + (active ? cp : 0);
     const int ld = nxh;                                    // row offsets inside a plane fit 32 bits
-    const LayoutCol<T> lay{c};
+    const typename YLayout<N, T>::type lay{c};
     const SyncCta sync;
 
     double2 v[E];
@@ -170,7 +190,7 @@ __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int compl
     const bool active = cp < nxh;
     double2 *base = w + (size_t)z * N * nxh + (active ? cp : 0);
     const int ld = nxh;                                    // row offsets inside a plane fit 32 bits
-    const LayoutCol<T> lay{c};
+    const typename YLayout<N, T>::type lay{c};
     const SyncCta sync;
     const bool cplx = complex_cols && cp > 0;
 
