@@ -81,7 +81,9 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
  *            caller.  u == f (exact aliasing, in place) is allowed; any other overlap is
  *            PP_ERR_INVALID_ARG.  f is not modified unless u == f.
  *   stream : a cudaStream_t passed as void* (NULL = the legacy default stream).
- * Asynchronous and stream-ordered: enqueues PP_NUM_KERNELS kernels on `stream`, never
+ * Asynchronous and stream-ordered: enqueues its kernels (pp_plan_launches_per_solve) on `stream` -- one
+ * small kernel of the long-line singular case runs on a plan-owned side stream, forked from and joined
+ * back into `stream` by events, so the ordering seen by the caller is the same -- never
  * allocates, never synchronises.  Launch errors are returned; execution errors surface at
  * the caller's next synchronisation.  All passes run in place in u: no N-sized workspace.
  */

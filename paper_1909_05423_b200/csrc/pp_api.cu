@@ -39,6 +39,8 @@ struct pp_plan {
     int xy_fusion;             // 1: x and y passes of a plane run as tasks of one kernel (pp_fused.cuh)
     int *fuse_sync;            // [1 + nz] ticket + per-plane completion counters
     double *hier_scratch;      // [4][nz / 256][nx ny]: interface values of the two-level z solve (long lines only)
+    cudaStream_t side;         // long singular lines only: the zero-mode line is solved beside the two-level passes
+    cudaEvent_t ev_fork, ev_join;
     cudaEvent_t ev[PP_NUM_KERNELS + 1];
 };
 
@@ -271,11 +273,21 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
         const dim3 grid((unsigned)((plane + hs.L - 1) / hs.L), (unsigned)nK);
         if (int rc = set_smem(zsolve_part_kernel<32, 1>, ds)) return rc;
         if (int rc = set_smem(zsolve_part_kernel<32, 2>, ds)) return rc;
+        if (p->singular) {
+            // the singular (0,0) line touches column 0 only, which the passes below never store and whose
+            // values they discard: it runs beside them on the plan's side stream (fork / join by events)
+            if (cudaEventRecord(p->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(p->side, p->ev_fork, 0) != cudaSuccess) {
+                cudaGetLastError();
+                return PP_ERR_CUDA;
+            }
+            zero_mode_long_kernel<<<1, 1024, 0, p->side>>>(w, plane, p->nz, p->scale);
+            if (cudaEventRecord(p->ev_join, p->side) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+        }
         zsolve_part_kernel<32, 1><<<grid, hs.L * hs.S, ds, st>>>(w, zp, hs.S, hs.L, h);
         zsolve_hier_interface_kernel<<<(unsigned)((plane + 63) / 64), 64, 0, st>>>(zp, h, ZP_HIER_ROWS, p->hier_scratch + 2 * slab,
                                                                              p->hier_scratch + 3 * slab);
         zsolve_part_kernel<32, 2><<<grid, hs.L * hs.S, ds, st>>>(w, zp, hs.S, hs.L, h);
-        if (p->singular) zero_mode_long_kernel<<<1, 1024, 0, st>>>(w, plane, p->nz, p->scale);
+        if (p->singular && cudaStreamWaitEvent(st, p->ev_join, 0) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
     } else if (p->bcz != PP_BC_PERIODIC) {
         // checkpoint table in shared memory: ceil(nz / CB) x TH doubles per CTA
 #define PP_ZT_LAUNCH(C, T)                                                                           \
@@ -313,6 +325,9 @@ void free_plan(pp_plan *p) {
     cudaFree(p->tw_x); cudaFree(p->tw_y); cudaFree(p->ptw_x); cudaFree(p->ptw_y);
     cudaFree(p->sx); cudaFree(p->sy); cudaFree(p->zero_scratch); cudaFree(p->host_stage); cudaFree(p->fuse_sync); cudaFree(p->hier_scratch);
     for (auto &e : p->ev) if (e) cudaEventDestroy(e);
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    if (p->ev_join) cudaEventDestroy(p->ev_join);
+    if (p->side) cudaStreamDestroy(p->side);
     cudaGetLastError();
     delete p;
 }
@@ -392,6 +407,14 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
         const size_t nb = sizeof(double) * 4 * (size_t)(nz / ZP_HIER_ROWS) * (size_t)nx * (size_t)ny;
         if (cudaMalloc((void **)&p->hier_scratch, nb) != cudaSuccess) { p->hier_scratch = nullptr; cudaGetLastError(); rc = PP_ERR_ALLOC; }
         else p->bytes += nb;
+    }
+    if (!rc && p->hier_scratch && p->singular) {
+        if (cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+            cudaGetLastError();
+            rc = PP_ERR_CUDA;
+        }
     }
     if (!rc) {
         const size_t nb = sizeof(int) * (size_t)(nz + 1);

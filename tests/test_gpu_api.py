@@ -109,7 +109,7 @@ def test_error_codes_on_device():
     del n
 
 
-@pytest.mark.parametrize("case", ["cfg1", "fused128", "long768"])
+@pytest.mark.parametrize("case", ["cfg1", "fused128", "long768", "long768-singular"])
 def test_pp_solve_is_graph_capturable(case):
     """pp_solve never allocates and never synchronises (include/pittpack_b200.h), so a solve can be
     captured into a CUDA graph and replayed -- what a time-stepping caller does with small grids,
@@ -122,7 +122,9 @@ def test_pp_solve_is_graph_capturable(case):
         w = wl.config2("PPN", "normal")
     else:
         shape = (768, 8, 16)
-        w = wl.Workload("long768", shape, (1.0 / 16, 1.0 / 8, 1.0 / 8), wl.parse_bc("NND"), wl.random_uniform(shape, 3))
+        combo = "NNN" if case.endswith("singular") else "NND"     # singular: the zero-mode kernel forks onto the side stream
+        f0 = wl.random_normal(shape, 3, zero_mean=True)
+        w = wl.Workload(case, shape, (1.0 / 16, 1.0 / 8, 1.0 / 8), wl.parse_bc(combo), f0)
     nz, ny, nx = w.shape
     plan = pp.Plan(nx, ny, nz, *w.h, w.bc)
     if case == "fused128":
