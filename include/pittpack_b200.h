@@ -127,7 +127,11 @@ int pp_plan_last_kernel_ms(pp_plan *plan, float *ms_out);
  *                    Neumann / Dirichlet z, nz = 256 m (2 <= m <= 64), where the same partition is
  *                    applied on two levels (super-segments of 256 rows, three kernels); otherwise
  *                    PP_ERR_UNSUPPORTED_SIZE and the plan is left unchanged.  PP_Z_SWEEP is
- *                    refused for nz > 4096.
+ *                    refused for nz > 4096.  The partitioned kernels tabulate segment
+ *                    determinants of magnitude up to (3 + max|s|)^R (R = 32 or 64 rows per
+ *                    segment, s the spectral shift dz^2 (lam_x/dx^2 + lam_y/dy^2)); grids so
+ *                    anisotropic that this could leave the fp64 range (dz/dx beyond ~90 with
+ *                    R = 64, ~17000 with R = 32) are solved by the two-sweep kernel instead.
  */
 enum { PP_Z_AUTO = 0, PP_Z_SWEEP = 1, PP_Z_PARTITION = 2 };
 int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm);

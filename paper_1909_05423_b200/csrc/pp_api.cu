@@ -36,6 +36,7 @@ struct pp_plan {
     int profiling;
     int have_times;
     int z_algorithm;           // PP_Z_AUTO / PP_Z_SWEEP / PP_Z_PARTITION
+    double bmax;               // largest |diagonal| of any z system, 3 + max |s| (range check of the partitioned kernels)
     int xy_fusion;             // 1: x and y passes of a plane run as tasks of one kernel (pp_fused.cuh)
     int *fuse_sync;            // [1 + nz] ticket + per-plane completion counters
     double *hier_scratch;      // [4][nz / 256][nx ny]: interface values of the two-level z solve (long lines only)
@@ -184,6 +185,14 @@ int run_y(const pp_plan *p, bool fwd, double *w, cudaStream_t st) {
 #undef CALL_Y
 }
 
+// The partitioned z kernels tabulate the leading minors q_0 .. q_R of a segment block, |q_R| <= bmax^R:
+// for grids so anisotropic (dz >> dx) that this could leave the fp64 range they are not used.
+bool zpart_range_ok(const pp_plan *p, int R) { return (double)R * std::log2(p->bmax) < 1000.0; }
+ZPartShape plan_zpart_shape(const pp_plan *p) {
+    const ZPartShape z = zpart_shape(p->nz);
+    return (z.R && zpart_range_ok(p, z.R)) ? z : ZPartShape{0, 0, 0};
+}
+
 // nx == ny in {128, 256, 512, 1024}: the sizes the fused x+y kernel is instantiated for
 bool fusion_supported(int nx, int ny) { return nx == ny && nx >= 128 && nx <= 1024; }
 
@@ -247,7 +256,7 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
 #define PP_Z_CB 16
 #endif
     const bool want_part = p->z_algorithm != PP_Z_SWEEP;
-    const ZPartShape zs = want_part ? zpart_shape(p->nz) : ZPartShape{0, 0, 0};
+    const ZPartShape zs = want_part ? plan_zpart_shape(p) : ZPartShape{0, 0, 0};
     if (zs.R) {
         // partitioned, register-resident solve: one HBM read + one write per unknown (pp_zpart.cuh)
         const bool cyc = p->bcz == PP_BC_PERIODIC;
@@ -395,15 +404,21 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
     if (!rc) rc = upload(&p->tw_y, tw, p->bytes);
     if (!rc) rc = upload(&p->ptw_y, ptw, p->bytes);
     const long double dz2 = (long double)dz * (long double)dz;
+    double smin = 0.0;
     make_shift(bc_x, nx, true, dz2 / ((long double)dx * (long double)dx), s);
+    { double m = 0.0; for (double v : s) m = v < m ? v : m; smin += m; }
     if (!rc) rc = upload(&p->sx, s, p->bytes);
     make_shift(bc_y, ny, false, dz2 / ((long double)dy * (long double)dy), s);
+    { double m = 0.0; for (double v : s) m = v < m ? v : m; smin += m; }
     if (!rc) rc = upload(&p->sy, s, p->bytes);
+    p->bmax = 3.0 - smin;
+    // lines beyond the two-sweep kernel's range need the two-level partition (segments of 32 rows)
+    if (!rc && nz > 64 * Z_MAX_CK && !zpart_range_ok(p, 32)) rc = PP_ERR_UNSUPPORTED_SIZE;
     if (!rc) {
         std::vector<double> z((size_t)nz, 0.0);
         rc = upload(&p->zero_scratch, z, p->bytes);
     }
-    if (!rc && long_ok && zpart_shape(nz).R == 0) {
+    if (!rc && long_ok && zpart_shape(nz).R == 0 && zpart_range_ok(p, 32)) {
         const size_t nb = sizeof(double) * 4 * (size_t)(nz / ZP_HIER_ROWS) * (size_t)nx * (size_t)ny;
         if (cudaMalloc((void **)&p->hier_scratch, nb) != cudaSuccess) { p->hier_scratch = nullptr; cudaGetLastError(); rc = PP_ERR_ALLOC; }
         else p->bytes += nb;
@@ -506,7 +521,7 @@ int pp_plan_set_profiling(pp_plan *plan, int enable) {
 int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm) {
     if (!plan) return PP_ERR_NULL;
     if (algorithm != PP_Z_AUTO && algorithm != PP_Z_SWEEP && algorithm != PP_Z_PARTITION) return PP_ERR_INVALID_ARG;
-    if (algorithm == PP_Z_PARTITION && zpart_shape(plan->nz).R == 0 && !plan->hier_scratch)
+    if (algorithm == PP_Z_PARTITION && plan_zpart_shape(plan).R == 0 && !plan->hier_scratch)
         return PP_ERR_UNSUPPORTED_SIZE;
     if (algorithm == PP_Z_SWEEP && plan->nz > 64 * Z_MAX_CK) return PP_ERR_UNSUPPORTED_SIZE;
     plan->z_algorithm = algorithm;
@@ -525,7 +540,7 @@ int pp_plan_launches_per_solve(const pp_plan *plan) {
     const bool fused = plan->xy_fusion && fusion_supported(plan->nx, plan->ny);
     int n = fused ? 2 : 4;                                        // x/y passes
     const bool want_part = plan->z_algorithm != PP_Z_SWEEP;
-    if (want_part && zpart_shape(plan->nz).R == 0 && plan->hier_scratch) n += 3 + (plan->singular ? 1 : 0);
+    if (want_part && plan_zpart_shape(plan).R == 0 && plan->hier_scratch) n += 3 + (plan->singular ? 1 : 0);
     else n += 1;
     return n;
 }

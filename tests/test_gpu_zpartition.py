@@ -56,6 +56,26 @@ def test_partition_large_shift_modes():
         assert e <= TOL, (combo, e)
 
 
+def test_extreme_anisotropy_falls_back_to_the_sweep():
+    """dz/dx = 256 with 64-row segments: the leading minors would reach |b|^64 ~ 1e360 and leave the fp64
+    range, so the plan must not use the partitioned kernel there (and must still be right)."""
+    import paper_1909_05423_b200 as pp
+    shape = (1024, 8, 16)
+    h = (1.0 / 4096, 1.0 / 4096, 1.0 / 16)
+    bc = wl.parse_bc("NND")
+    f = wl.random_uniform(shape, 11)
+    ref = po.solve(f, h, bc)
+    assert rel_err(gpu_solve(f, h, bc), ref) <= TOL
+    plan = pp.Plan(16, 8, 1024, *h, bc)
+    with pytest.raises(pp.PittPackError):
+        plan.set_z_algorithm("partition")
+    plan.destroy()
+    # the same grid with 32-row segments (nz = 256) is inside the range
+    shape = (256, 8, 16)
+    f = wl.random_uniform(shape, 12)
+    assert rel_err(gpu_solve(f, h, bc, z_algorithm="partition"), po.solve(f, h, bc)) <= TOL
+
+
 def test_partition_refused_where_it_does_not_apply():
     import paper_1909_05423_b200 as pp
     for nz, combo in ((48, "PPN"), (768, "PPP"), (100, "DDD")):
