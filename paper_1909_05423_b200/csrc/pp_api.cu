@@ -194,7 +194,7 @@ ZPartShape plan_zpart_shape(const pp_plan *p) {
 }
 
 // nx == ny in {128, 256, 512, 1024}: the sizes the fused x+y kernel is instantiated for
-bool fusion_supported(int nx, int ny) { return nx == ny && nx >= 128 && nx <= 1024; }
+bool fusion_supported(int nx, int ny) { return nx == ny && nx >= 128 && nx <= 1024 && (nx & (nx - 1)) == 0; }
 
 #ifndef PP_FUSE_LAG
 #define PP_FUSE_LAG 0          // 0: derived from the number of resident CTAs

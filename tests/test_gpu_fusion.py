@@ -61,7 +61,7 @@ def test_fused_in_place_and_repeated():
 
 def test_fusion_refused_where_it_does_not_apply():
     import paper_1909_05423_b200 as pp
-    for nx, ny in ((64, 64), (256, 128), (2048, 2048)):
+    for nx, ny in ((64, 64), (256, 128), (2048, 2048), (384, 384)):
         plan = pp.Plan(nx, ny, 4, 0.1, 0.1, 0.1, "PPN")
         with pytest.raises(pp.PittPackError):
             plan.set_xy_fusion(True)
