@@ -149,6 +149,13 @@ int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm);
 int pp_plan_set_xy_fusion(pp_plan *plan, int enable);
 
 /*
+ * 1 if pp_plan_create accepts this grid (see its size rules), else 0.  Host-only: needs no device.
+ * (Spacing-dependent refusals -- lines longer than 4096 on extremely anisotropic grids -- are not
+ * covered: they need dx, dy, dz.)
+ */
+int pp_size_supported(int nx, int ny, int nz, int bc_z);
+
+/*
  * Number of kernels one pp_solve launches with the plan's current settings: 5 by default (PP_K_*),
  * 3 with x+y fusion, +2 (+1 more when the problem is singular) when the z solve is the two-level
  * partition for long lines.  0 for a NULL plan.

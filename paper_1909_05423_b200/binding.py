@@ -21,7 +21,7 @@ KERNEL_NAMES = ("x_fwd", "y_fwd", "z_solve", "y_inv", "x_inv")
 
 EXPORTS = (
     "pp_plan_create", "pp_solve", "pp_solve_host", "pp_plan_destroy", "pp_plan_workspace_bytes",
-    "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_plan_set_xy_fusion", "pp_plan_launches_per_solve", "pp_strerror", "pp_version",
+    "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_plan_set_xy_fusion", "pp_plan_launches_per_solve", "pp_size_supported", "pp_strerror", "pp_version",
 )
 PP_Z_AUTO, PP_Z_SWEEP, PP_Z_PARTITION = 0, 1, 2
 
@@ -65,6 +65,8 @@ def lib() -> ctypes.CDLL:
     L.pp_plan_set_xy_fusion.restype = i32
     L.pp_plan_launches_per_solve.argtypes = [vp]
     L.pp_plan_launches_per_solve.restype = i32
+    L.pp_size_supported.argtypes = [i32, i32, i32, i32]
+    L.pp_size_supported.restype = i32
     L.pp_strerror.argtypes = [i32]
     L.pp_strerror.restype = ctypes.c_char_p
     L.pp_version.argtypes = []
@@ -121,6 +123,10 @@ def pp_plan_set_xy_fusion(plan, enable):
 
 def pp_plan_launches_per_solve(plan):
     return int(lib().pp_plan_launches_per_solve(ctypes.c_void_p(plan)))
+
+
+def pp_size_supported(nx, ny, nz, bc_z):
+    return bool(lib().pp_size_supported(int(nx), int(ny), int(nz), int(bc_z)))
 
 
 def strerror(status: int) -> str:

@@ -535,6 +535,12 @@ int pp_plan_set_xy_fusion(pp_plan *plan, int enable) {
     return PP_SUCCESS;
 }
 
+int pp_size_supported(int nx, int ny, int nz, int bc_z) {
+    if (bc_z != PP_BC_PERIODIC && bc_z != PP_BC_NEUMANN && bc_z != PP_BC_DIRICHLET) return 0;
+    const bool long_ok = bc_z != PP_BC_PERIODIC && zpart_hier_ok(nz);
+    return (length_supported(nx) && length_supported(ny) && nz >= 2 && (nz <= 64 * Z_MAX_CK || long_ok)) ? 1 : 0;
+}
+
 int pp_plan_launches_per_solve(const pp_plan *plan) {
     if (!plan) return 0;
     const bool fused = plan->xy_fusion && fusion_supported(plan->nx, plan->ny);

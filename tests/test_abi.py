@@ -88,3 +88,22 @@ def test_product_path_does_not_import_the_oracle():
             if name.endswith((".py", ".cu", ".cuh", ".h")):
                 text = open(os.path.join(dirpath, name)).read()
                 assert not pat.search(text), name
+
+
+def test_size_rules_host_side():
+    """pp_size_supported needs no device: 2^k in [4, 2048], 3*2^k in [48, 1536], 5*2^k in [80, 1280];
+    nz in [2, 4096], or 256 m <= 16384 with non-periodic z."""
+    import paper_1909_05423_b200 as pp
+    ok = pp.binding.pp_size_supported
+    good = [4, 8, 512, 2048, 48, 96, 192, 384, 768, 1536, 80, 160, 320, 640, 1280]
+    bad = [0, 2, 3, 6, 12, 24, 36, 40, 56, 112, 144, 4096, 3072, 2560, 100, 1000]
+    for n in good:
+        assert ok(n, 64, 32, 1) and ok(64, n, 32, 2), n
+    for n in bad:
+        assert not ok(n, 64, 32, 1) and not ok(64, n, 32, 0), n
+    assert ok(64, 64, 2, 0) and ok(64, 64, 4096, 0) and not ok(64, 64, 1, 0)
+    assert ok(64, 64, 16384, 1) and ok(48, 48, 8192, 2)
+    assert not ok(64, 64, 16384, 0)              # long lines: non-periodic z only
+    assert not ok(64, 64, 8192 + 32, 1)          # ... in multiples of 256
+    assert not ok(64, 64, 32768, 1)              # ... up to 16384
+    assert not ok(64, 64, 64, 7)                 # unknown boundary condition
