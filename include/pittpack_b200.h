@@ -149,6 +149,19 @@ int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm);
 int pp_plan_set_xy_fusion(pp_plan *plan, int enable);
 
 /*
+ * Which solution of a singular problem (all three axes periodic or Neumann) is returned.  f is
+ * projected to zero mean either way (second alternative); the solution is then fixed
+ * up to a constant:
+ *   PP_NULL_ZERO_MEAN  : zero volume mean, u = pinv(A) f (the default; what the oracle returns).
+ *   PP_NULL_PIN_PLANE0 : the mean of the z = 0 plane is zero -- the paper's default ("keeping the
+ *                        corner value which is the mean of the function at z=0 plane fixed",
+ *                        PAPER.md:533).  Differs from the first by the constant mean_xy u(:,:,0).
+ * No effect on non-singular plans.
+ */
+enum { PP_NULL_ZERO_MEAN = 0, PP_NULL_PIN_PLANE0 = 1 };
+int pp_plan_set_null_space(pp_plan *plan, int convention);
+
+/*
  * 1 if pp_plan_create accepts this grid (see its size rules), else 0.  Host-only: needs no device.
  * (Spacing-dependent refusals -- lines longer than 4096 on extremely anisotropic grids -- are not
  * covered: they need dx, dy, dz.)

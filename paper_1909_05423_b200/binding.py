@@ -21,9 +21,10 @@ KERNEL_NAMES = ("x_fwd", "y_fwd", "z_solve", "y_inv", "x_inv")
 
 EXPORTS = (
     "pp_plan_create", "pp_solve", "pp_solve_host", "pp_plan_destroy", "pp_plan_workspace_bytes",
-    "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_plan_set_xy_fusion", "pp_plan_launches_per_solve", "pp_size_supported", "pp_strerror", "pp_version",
+    "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_plan_set_xy_fusion", "pp_plan_launches_per_solve", "pp_size_supported", "pp_plan_set_null_space", "pp_strerror", "pp_version",
 )
 PP_Z_AUTO, PP_Z_SWEEP, PP_Z_PARTITION = 0, 1, 2
+PP_NULL_ZERO_MEAN, PP_NULL_PIN_PLANE0 = 0, 1
 
 _lib = None
 
@@ -67,6 +68,8 @@ def lib() -> ctypes.CDLL:
     L.pp_plan_launches_per_solve.restype = i32
     L.pp_size_supported.argtypes = [i32, i32, i32, i32]
     L.pp_size_supported.restype = i32
+    L.pp_plan_set_null_space.argtypes = [vp, i32]
+    L.pp_plan_set_null_space.restype = i32
     L.pp_strerror.argtypes = [i32]
     L.pp_strerror.restype = ctypes.c_char_p
     L.pp_version.argtypes = []
@@ -127,6 +130,10 @@ def pp_plan_launches_per_solve(plan):
 
 def pp_size_supported(nx, ny, nz, bc_z):
     return bool(lib().pp_size_supported(int(nx), int(ny), int(nz), int(bc_z)))
+
+
+def pp_plan_set_null_space(plan, convention):
+    return lib().pp_plan_set_null_space(ctypes.c_void_p(plan), int(convention))
 
 
 def strerror(status: int) -> str:
@@ -215,6 +222,13 @@ class Plan:
         st = pp_plan_set_xy_fusion(self.handle, enable)
         if st != PP_SUCCESS:
             raise PittPackError(st, "pp_plan_set_xy_fusion")
+
+    def set_null_space(self, convention):
+        """'zero_mean' | 'pin_plane0' (or a PP_NULL_* value)."""
+        c = {"zero_mean": PP_NULL_ZERO_MEAN, "pin_plane0": PP_NULL_PIN_PLANE0}.get(convention, convention)
+        st = pp_plan_set_null_space(self.handle, c)
+        if st != PP_SUCCESS:
+            raise PittPackError(st, "pp_plan_set_null_space")
 
     @property
     def launches_per_solve(self):

@@ -37,6 +37,7 @@ struct pp_plan {
     int have_times;
     int z_algorithm;           // PP_Z_AUTO / PP_Z_SWEEP / PP_Z_PARTITION
     double bmax;               // largest |diagonal| of any z system, 3 + max |s| (range check of the partitioned kernels)
+    int null_space;            // PP_NULL_ZERO_MEAN / PP_NULL_PIN_PLANE0 (singular problems only)
     int xy_fusion;             // 1: x and y passes of a plane run as tasks of one kernel (pp_fused.cuh)
     int *fuse_sync;            // [1 + nz] ticket + per-plane completion counters
     double *hier_scratch;      // [4][nz / 256][nx ny]: interface values of the two-level z solve (long lines only)
@@ -244,7 +245,7 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
     ZParams zp;
     zp.nx = p->nx; zp.ny = p->ny; zp.nz = p->nz;
     zp.bcz = p->bcz;
-    zp.singular = p->singular;
+    zp.singular = p->singular ? (p->null_space == PP_NULL_PIN_PLANE0 ? 2 : 1) : 0;
     zp.scale = p->scale;
     zp.sx = p->sx; zp.sy = p->sy;
     zp.zero_scratch = p->zero_scratch;
@@ -289,7 +290,7 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
                 cudaGetLastError();
                 return PP_ERR_CUDA;
             }
-            zero_mode_long_kernel<<<1, 1024, 0, p->side>>>(w, plane, p->nz, p->scale);
+            zero_mode_long_kernel<<<1, 1024, 0, p->side>>>(w, plane, p->nz, p->scale, p->null_space == PP_NULL_PIN_PLANE0);
             if (cudaEventRecord(p->ev_join, p->side) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
         }
         zsolve_part_kernel<32, 1><<<grid, hs.L * hs.S, ds, st>>>(w, zp, hs.S, hs.L, h);
@@ -532,6 +533,13 @@ int pp_plan_set_xy_fusion(pp_plan *plan, int enable) {
     if (!plan) return PP_ERR_NULL;
     if (enable && !fusion_supported(plan->nx, plan->ny)) return PP_ERR_UNSUPPORTED_SIZE;
     plan->xy_fusion = enable ? 1 : 0;
+    return PP_SUCCESS;
+}
+
+int pp_plan_set_null_space(pp_plan *plan, int convention) {
+    if (!plan) return PP_ERR_NULL;
+    if (convention != PP_NULL_ZERO_MEAN && convention != PP_NULL_PIN_PLANE0) return PP_ERR_INVALID_ARG;
+    plan->null_space = convention;
     return PP_SUCCESS;
 }
 

@@ -378,7 +378,7 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
     }
     // the warp that owns element 0 solves the singular line together (its line was never stored above)
     // (long lines: zero_mode_long_kernel does it with a whole CTA)
-    if (MODE == 0 && p.singular && blockIdx.x == 0 && threadIdx.x < 32) zero_mode_line(w, plane, p.nz, p.bcz, p.scale, p.zero_scratch);
+    if (MODE == 0 && p.singular && blockIdx.x == 0 && threadIdx.x < 32) zero_mode_line(w, plane, p.nz, p.bcz, p.scale, p.zero_scratch, p.singular == 2);
 }
 
 // Couples the super-segments of every line (see ZHier): one thread per mode.  The super-segment block
@@ -493,7 +493,7 @@ __device__ __forceinline__ double zp_block_excl_scan(double v, double *red, doub
 }
 
 __global__ void __launch_bounds__(1024, 1)
-zero_mode_long_kernel(double *col, size_t plane, int nz, double scale) {
+zero_mode_long_kernel(double *col, size_t plane, int nz, double scale, int pin_plane0) {
     __shared__ double red[32];
     constexpr int C = 16;
     const int c = (nz + (int)blockDim.x - 1) / (int)blockDim.x;        // <= C
@@ -537,7 +537,7 @@ zero_mode_long_kernel(double *col, size_t plane, int nz, double scale) {
     }
     double xtot;
     zp_block_excl_scan(xs, red, xtot);
-    const double xmean = xtot / nz;
+    const double xmean = pin_plane0 ? 0.0 : xtot / nz;
 #pragma unroll
     for (int i = 0; i < C; ++i)
         if (i < c && k0 + i < k1) col[(size_t)(k0 + i) * plane] = v[i] - xmean;

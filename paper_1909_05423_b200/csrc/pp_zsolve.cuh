@@ -31,7 +31,8 @@ namespace pp {
 struct ZParams {
     int nx, ny, nz;
     int bcz;
-    int singular;            // 1: element 0 (kx = ky = 0) is the singular zero mode
+    int singular;            // 1, 2: element 0 (kx = ky = 0) is the singular zero mode; 2: return the solution whose
+                             // z = 0 plane has zero mean (the paper's default) instead of zero volume mean
     double scale;            // dz^2 / (nx ny): rhs scaling incl. the inverse-transform normalisation
     const double *sx;        // [nx]  dz^2 lam_x(kx(ix)) / dx^2
     const double *sy;        // [ny]  dz^2 lam_y(ky(j))  / dy^2
@@ -105,7 +106,8 @@ __device__ __forceinline__ double warp_excl_scan(double v, int lane) {
     return inc - v;
 }
 
-__device__ __noinline__ void zero_mode_line(double *col, size_t plane, int nz, int bcz, double scale, double *tmp) {
+__device__ __noinline__ void zero_mode_line(double *col, size_t plane, int nz, int bcz, double scale, double *tmp,
+                                            bool pin_plane0) {
     const int lane = threadIdx.x & 31;
     const int c = (nz + 31) / 32;
     const int k0 = min(lane * c, nz), k1 = min(k0 + c, nz);
@@ -140,7 +142,8 @@ __device__ __noinline__ void zero_mode_line(double *col, size_t plane, int nz, i
     double run = warp_excl_scan(dt, lane);
     double xs = 0.0;
     for (int k = max(k0, 1); k < k1; ++k) { run += tmp[k]; tmp[k] = run; xs += run; }
-    const double xmean = warp_sum(xs) / nz;                   // x_0 = 0 contributes nothing
+    // x_0 = 0 contributes nothing; with the plane-0 convention the pinned x_0 = 0 already is the answer
+    const double xmean = pin_plane0 ? 0.0 : warp_sum(xs) / nz;
     for (int k = k0; k < k1; ++k) col[(size_t)k * plane] = ((k == 0) ? 0.0 : tmp[k]) - xmean;
 }
 
@@ -317,7 +320,7 @@ zsolve_thomas_kernel(double *w, ZParams p) {
         }
     }
     // the warp that owns element 0 solves the singular line together (block 0, warp 0: all lanes alive)
-    if (p.singular && e < 32) zero_mode_line(w, plane, nz, p.bcz, scale, p.zero_scratch);
+    if (p.singular && e < 32) zero_mode_line(w, plane, nz, p.bcz, scale, p.zero_scratch, p.singular == 2);
 }
 
 // Periodic in z: Sherman-Morrison, "two solves".  With gamma = -b:
@@ -401,7 +404,7 @@ zsolve_cyclic_kernel(double *w, ZParams p) {
         if (sweep == 0) fac = (x + xlast / gamma) / (1.0 + q + qlast / gamma);
     }
     // the warp that owns element 0 solves the singular line together (block 0, warp 0: all lanes alive)
-    if (p.singular && e < 32) zero_mode_line(w, plane, nz, p.bcz, scale, p.zero_scratch);
+    if (p.singular && e < 32) zero_mode_line(w, plane, nz, p.bcz, scale, p.zero_scratch, p.singular == 2);
 }
 
 }  // namespace pp

@@ -146,3 +146,26 @@ def test_pp_solve_is_graph_capturable(case):
     assert torch.equal(u, ref)
     assert rel_err(u.cpu().numpy(), po.solve(w.f, w.h, w.bc)) <= TOL
     plan.destroy()
+
+
+@pytest.mark.parametrize("combo,shape", [("PPN", (64, 16, 32)), ("NNN", (40, 8, 16)), ("PPP", (64, 16, 16)),
+                                         ("NNP", (17, 8, 16)), ("PPN", (768, 8, 16))])
+def test_pinned_plane_null_space(combo, shape):
+    """The paper's own convention for singular problems: the mean of the z = 0 plane is kept
+    at zero.  It differs from the zero-mean solution (the oracle's, R11) by a constant only."""
+    import torch
+    import paper_1909_05423_b200 as pp
+    bc = wl.parse_bc(combo)
+    nz, ny, nx = shape
+    h = (1.0 / nx, 1.0 / ny, 2.0 / nz)
+    f = wl.random_normal(shape, 900 + nz, zero_mean=True)
+    ref = po.solve(f, h, bc)
+    plan = pp.Plan(nx, ny, nz, *h, bc)
+    plan.set_null_space("pin_plane0")
+    u = plan.solve(torch.from_numpy(f).cuda()).cpu().numpy()
+    assert abs(u[0].mean()) <= 1e-13 * np.abs(u).max()
+    assert rel_err(u, ref - ref[0].mean()) <= TOL
+    plan.set_null_space("zero_mean")
+    u0 = plan.solve(torch.from_numpy(f).cuda()).cpu().numpy()
+    assert rel_err(u0, ref) <= TOL
+    plan.destroy()
