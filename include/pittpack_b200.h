@@ -149,6 +149,20 @@ int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm);
 int pp_plan_set_xy_fusion(pp_plan *plan, int enable);
 
 /*
+ * Non-homogeneous Dirichlet face values, moved to the right-hand side as PAPER.md:163 prescribes for
+ * a ghost cell extrapolated linearly through the face value:  f[boundary cell] -= 2 g / h^2.
+ * Call it on f before pp_solve (which solves the homogeneous problem); cells on an edge or a corner
+ * receive every face's term.
+ *   f                    : DEVICE pointer, nx*ny*nz doubles, modified in place.
+ *   gx_lo, gx_hi         : DEVICE arrays [nz][ny] of values on the faces x = 0 / x = nx dx, or NULL.
+ *   gy_lo, gy_hi         : [nz][nx] on y = 0 / y = ny dy, or NULL.   gz_lo, gz_hi : [ny][nx], or NULL.
+ * A non-NULL face of an axis that is not Dirichlet is PP_ERR_INVALID_ARG.  Stream-ordered, no sync.
+ */
+int pp_fold_dirichlet(const pp_plan *plan, double *f, const double *gx_lo, const double *gx_hi,
+                      const double *gy_lo, const double *gy_hi, const double *gz_lo, const double *gz_hi,
+                      void *stream);
+
+/*
  * Which solution of a singular problem (all three axes periodic or Neumann) is returned.  f is
  * projected to zero mean either way (second alternative); the solution is then fixed
  * up to a constant:

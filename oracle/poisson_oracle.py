@@ -294,6 +294,34 @@ def solve(f: np.ndarray, h, bc, zdtype=np.float64) -> np.ndarray:
 # --------------------------------------------------------------------------------------
 # the operator itself, for residual checks and brute force
 # --------------------------------------------------------------------------------------
+def fold_dirichlet(f: np.ndarray, h, bc, faces: dict) -> np.ndarray:
+    """Non-homogeneous Dirichlet values moved to the right-hand side: with the ghost cell
+    linearly extrapolated through the face value g, u_ghost = 2 g - u_0, the stencil of a boundary cell
+    reads (u_1 - 3 u_0)/h^2 + 2 g/h^2 = f_0, i.e. the homogeneous operator with  f_0 <- f_0 - 2 g/h^2.
+
+    ``faces`` maps (axis, side) -- axis in 'xyz', side 0 (lower face) or 1 (upper face) -- to the array of
+    face values: shape (nz, ny) for x faces, (nz, nx) for y faces, (ny, nx) for z faces.  Returns a new
+    array; ``f`` has shape (nz, ny, nx).  Every axis named must be Dirichlet."""
+    out = np.array(f, dtype=np.float64, copy=True)
+    nz, ny, nx = out.shape
+    for (axis, side), g in faces.items():
+        a = "xyz".index(axis)
+        if bc[a] != DIRICHLET:
+            raise ValueError(f"axis {axis} is not Dirichlet")
+        c = 2.0 / (h[a] * h[a])
+        g = np.asarray(g, dtype=np.float64)
+        if axis == "x":
+            assert g.shape == (nz, ny)
+            out[:, :, nx - 1 if side else 0] -= c * g
+        elif axis == "y":
+            assert g.shape == (nz, nx)
+            out[:, ny - 1 if side else 0, :] -= c * g
+        else:
+            assert g.shape == (ny, nx)
+            out[nz - 1 if side else 0, :, :] -= c * g
+    return out
+
+
 def apply_A(u: np.ndarray, h, bc) -> np.ndarray:
     """``A u`` by the 7-point stencil of eq. 3 with the homogeneous boundary
     rows of :func:`lap1d`, written with shifted slices (no matrix)."""

@@ -21,7 +21,7 @@ KERNEL_NAMES = ("x_fwd", "y_fwd", "z_solve", "y_inv", "x_inv")
 
 EXPORTS = (
     "pp_plan_create", "pp_solve", "pp_solve_host", "pp_plan_destroy", "pp_plan_workspace_bytes",
-    "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_plan_set_xy_fusion", "pp_plan_launches_per_solve", "pp_size_supported", "pp_plan_set_null_space", "pp_strerror", "pp_version",
+    "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_plan_set_xy_fusion", "pp_plan_launches_per_solve", "pp_size_supported", "pp_plan_set_null_space", "pp_fold_dirichlet", "pp_strerror", "pp_version",
 )
 PP_Z_AUTO, PP_Z_SWEEP, PP_Z_PARTITION = 0, 1, 2
 PP_NULL_ZERO_MEAN, PP_NULL_PIN_PLANE0 = 0, 1
@@ -70,6 +70,8 @@ def lib() -> ctypes.CDLL:
     L.pp_size_supported.restype = i32
     L.pp_plan_set_null_space.argtypes = [vp, i32]
     L.pp_plan_set_null_space.restype = i32
+    L.pp_fold_dirichlet.argtypes = [vp] * 9
+    L.pp_fold_dirichlet.restype = i32
     L.pp_strerror.argtypes = [i32]
     L.pp_strerror.restype = ctypes.c_char_p
     L.pp_version.argtypes = []
@@ -134,6 +136,12 @@ def pp_size_supported(nx, ny, nz, bc_z):
 
 def pp_plan_set_null_space(plan, convention):
     return lib().pp_plan_set_null_space(ctypes.c_void_p(plan), int(convention))
+
+
+def pp_fold_dirichlet(plan, f_ptr, gx_lo=0, gx_hi=0, gy_lo=0, gy_hi=0, gz_lo=0, gz_hi=0, stream=0):
+    """Face pointers are device addresses (0 = no face)."""
+    args = [ctypes.c_void_p(int(a)) for a in (plan, f_ptr, gx_lo, gx_hi, gy_lo, gy_hi, gz_lo, gz_hi, stream)]
+    return lib().pp_fold_dirichlet(*args)
 
 
 def strerror(status: int) -> str:
@@ -222,6 +230,25 @@ class Plan:
         st = pp_plan_set_xy_fusion(self.handle, enable)
         if st != PP_SUCCESS:
             raise PittPackError(st, "pp_plan_set_xy_fusion")
+
+    def fold_dirichlet(self, f, faces, stream=None):
+        """``faces``: {('x'|'y'|'z', 0|1): float64 CUDA tensor of face values}; f is modified in place."""
+        import torch
+        self._check(f, "f")
+        nz, ny, nx = self.shape
+        want = {"x": (nz, ny), "y": (nz, nx), "z": (ny, nx)}
+        ptr = {}
+        for (axis, side), g in faces.items():
+            if not (isinstance(g, torch.Tensor) and g.is_cuda and g.dtype == torch.float64 and g.is_contiguous()
+                    and tuple(g.shape) == want[axis]):
+                raise ValueError(f"face {axis}{side}: need a contiguous float64 CUDA tensor of shape {want[axis]}")
+            ptr[(axis, side)] = g.data_ptr()
+        s = torch.cuda.current_stream(f.device) if stream is None else stream
+        st = pp_fold_dirichlet(self.handle, f.data_ptr(), *(ptr.get((a, k), 0) for a in "xyz" for k in (0, 1)),
+                               stream=s.cuda_stream)
+        if st != PP_SUCCESS:
+            raise PittPackError(st, "pp_fold_dirichlet")
+        return f
 
     def set_null_space(self, convention):
         """'zero_mean' | 'pin_plane0' (or a PP_NULL_* value)."""

@@ -194,6 +194,17 @@ ZPartShape plan_zpart_shape(const pp_plan *p) {
     return (z.R && zpart_range_ok(p, z.R)) ? z : ZPartShape{0, 0, 0};
 }
 
+// Non-homogeneous Dirichlet face values moved to the right-hand side:
+//   f[offset + i sf + j ss] -= coef g[j nf + i],   coef = 2 / h^2,  (i, j) over one face of nf x ns cells
+__global__ void fold_face_kernel(double *f, const double *__restrict__ g, int nf, int ns, long long sf, long long ss,
+                                 long long offset, double coef) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (i < nf && j < ns) {
+        double *cell = f + offset + i * sf + j * ss;
+        *cell = *cell - __dmul_rn(coef, g[(long long)j * nf + i]);      // two roundings, like the oracle (no FMA)
+    }
+}
+
 // nx == ny in {128, 256, 512, 1024}: the sizes the fused x+y kernel is instantiated for
 bool fusion_supported(int nx, int ny) { return nx == ny && nx >= 128 && nx <= 1024 && (nx & (nx - 1)) == 0; }
 
@@ -534,6 +545,28 @@ int pp_plan_set_xy_fusion(pp_plan *plan, int enable) {
     if (enable && !fusion_supported(plan->nx, plan->ny)) return PP_ERR_UNSUPPORTED_SIZE;
     plan->xy_fusion = enable ? 1 : 0;
     return PP_SUCCESS;
+}
+
+int pp_fold_dirichlet(const pp_plan *plan, double *f, const double *gx_lo, const double *gx_hi, const double *gy_lo,
+                      const double *gy_hi, const double *gz_lo, const double *gz_hi, void *stream) {
+    if (!plan || !f) return PP_ERR_NULL;
+    if (((gx_lo || gx_hi) && plan->bcx != PP_BC_DIRICHLET) || ((gy_lo || gy_hi) && plan->bcy != PP_BC_DIRICHLET) ||
+        ((gz_lo || gz_hi) && plan->bcz != PP_BC_DIRICHLET))
+        return PP_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long nx = plan->nx, ny = plan->ny, nz = plan->nz;
+    auto fold = [&](const double *g, long long nf, long long ns, long long sf, long long ss, long long offset, double h) {
+        if (!g) return;
+        const dim3 grid((unsigned)((nf + 127) / 128), (unsigned)ns);
+        fold_face_kernel<<<grid, 128, 0, st>>>(f, g, (int)nf, (int)ns, sf, ss, offset, 2.0 / (h * h));
+    };
+    fold(gx_lo, ny, nz, nx, nx * ny, 0, plan->dx);                        // g[k][j] -> cell (0, j, k)
+    fold(gx_hi, ny, nz, nx, nx * ny, nx - 1, plan->dx);
+    fold(gy_lo, nx, nz, 1, nx * ny, 0, plan->dy);                         // g[k][i] -> cell (i, 0, k)
+    fold(gy_hi, nx, nz, 1, nx * ny, (ny - 1) * nx, plan->dy);
+    fold(gz_lo, nx, ny, 1, nx, 0, plan->dz);                              // g[j][i] -> cell (i, j, 0)
+    fold(gz_hi, nx, ny, 1, nx, (nz - 1) * nx * ny, plan->dz);
+    return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
 }
 
 int pp_plan_set_null_space(pp_plan *plan, int convention) {

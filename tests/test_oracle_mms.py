@@ -119,3 +119,34 @@ def test_fig16_case():
     uh = po.solve(f, h, bc)
     e = float(np.sqrt(np.mean((uh - u) ** 2)))
     assert abs(e - closed_form_error(bc, n, omega)) <= 1e-9 * e + 1e-15
+
+
+def test_nonhomogeneous_dirichlet_faces_converge_second_order():
+    """face values folded into the source, f_0 -= 2 g / h^2.  A solution that is non-zero
+    (and different) on all six faces; a wrong sign, a wrong factor or a swapped face breaks the order."""
+    def exact(x, y, z):
+        return np.cos(1.3 * x + 0.2) * np.exp(0.7 * y) * (1.0 + 0.5 * z * z) + 0.3 * x * z
+
+    def lap(x, y, z):
+        core = np.cos(1.3 * x + 0.2) * np.exp(0.7 * y)
+        return core * ((-1.69 + 0.49) * (1.0 + 0.5 * z * z) + 1.0)
+
+    errs = []
+    for n in (16, 32, 64):
+        hh = 1.0 / n
+        c = (np.arange(n) + 0.5) * hh
+        Z, Y, X = np.meshgrid(c, c, c, indexing="ij")
+        f = lap(X, Y, Z)
+        faces = {}
+        for side, pos in ((0, 0.0), (1, 1.0)):
+            zz, yy = np.meshgrid(c, c, indexing="ij")
+            faces[("x", side)] = exact(pos, yy, zz)                     # (nz, ny)
+            zz, xx = np.meshgrid(c, c, indexing="ij")
+            faces[("y", side)] = exact(xx, pos, zz)                     # (nz, nx)
+            yy, xx = np.meshgrid(c, c, indexing="ij")
+            faces[("z", side)] = exact(xx, yy, pos)                     # (ny, nx)
+        bc = (po.DIRICHLET,) * 3
+        u = po.solve(po.fold_dirichlet(f, (hh,) * 3, bc, faces), (hh,) * 3, bc)
+        errs.append(float(np.sqrt(np.mean((u - exact(X, Y, Z)) ** 2))))
+    for coarse, fine in zip(errs[:-1], errs[1:]):
+        assert abs(coarse / fine - 4.0) <= 0.3, errs
