@@ -97,6 +97,15 @@ int pp_solve(const pp_plan *plan, const double *f, double *u, void *stream);
  */
 int pp_solve_host(pp_plan *plan, const double *f_host, double *u_host, void *stream);
 
+/*
+ * nbatch independent solves with HOST buffers: right-hand side i is the i-th block of nx*ny*nz doubles of
+ * f_host, its solution the i-th block of u_host (pinned memory recommended; the two may be the same buffer).
+ * The copy-in of right-hand side i+1 and the copy-out of solution i-1 run beside the solve of i (two
+ * plan-owned copy streams, a ring of three plan-owned device buffers, allocated on first use), so a long
+ * batch costs one PCIe direction per solve instead of two.  Synchronises before returning.
+ */
+int pp_solve_host_batch(pp_plan *plan, const double *f_host, double *u_host, int nbatch, void *stream);
+
 /* Free the plan and everything it owns.  NULL is a no-op returning PP_SUCCESS. */
 int pp_plan_destroy(pp_plan *plan);
 

@@ -20,7 +20,7 @@ PP_NUM_KERNELS = 5
 KERNEL_NAMES = ("x_fwd", "y_fwd", "z_solve", "y_inv", "x_inv")
 
 EXPORTS = (
-    "pp_plan_create", "pp_solve", "pp_solve_host", "pp_plan_destroy", "pp_plan_workspace_bytes",
+    "pp_plan_create", "pp_solve", "pp_solve_host", "pp_solve_host_batch", "pp_plan_destroy", "pp_plan_workspace_bytes",
     "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_plan_set_xy_fusion", "pp_plan_launches_per_solve", "pp_size_supported", "pp_plan_set_null_space", "pp_fold_dirichlet", "pp_strerror", "pp_version",
 )
 PP_Z_AUTO, PP_Z_SWEEP, PP_Z_PARTITION = 0, 1, 2
@@ -52,6 +52,8 @@ def lib() -> ctypes.CDLL:
     L.pp_solve.restype = i32
     L.pp_solve_host.argtypes = [vp, vp, vp, vp]
     L.pp_solve_host.restype = i32
+    L.pp_solve_host_batch.argtypes = [vp, vp, vp, i32, vp]
+    L.pp_solve_host_batch.restype = i32
     L.pp_plan_destroy.argtypes = [vp]
     L.pp_plan_destroy.restype = i32
     L.pp_plan_workspace_bytes.argtypes = [vp]
@@ -97,6 +99,11 @@ def pp_solve(plan, f_ptr, u_ptr, stream=0):
 def pp_solve_host(plan, f_ptr, u_ptr, stream=0):
     return lib().pp_solve_host(ctypes.c_void_p(plan), ctypes.c_void_p(f_ptr), ctypes.c_void_p(u_ptr),
                                ctypes.c_void_p(stream))
+
+
+def pp_solve_host_batch(plan, f_ptr, u_ptr, nbatch, stream=0):
+    return lib().pp_solve_host_batch(ctypes.c_void_p(plan), ctypes.c_void_p(f_ptr), ctypes.c_void_p(u_ptr), int(nbatch),
+                                     ctypes.c_void_p(stream))
 
 
 def pp_plan_destroy(plan):
@@ -206,6 +213,19 @@ class Plan:
         st = pp_solve_host(self.handle, f_host.data_ptr(), u_host.data_ptr(), s.cuda_stream)
         if st != PP_SUCCESS:
             raise PittPackError(st, "pp_solve_host")
+        return u_host
+
+    def solve_host_batch(self, f_host, u_host, stream=None):
+        """f_host, u_host: contiguous float64 CPU tensors of shape (nbatch, nz, ny, nx), pinned recommended."""
+        import torch
+        for t, name in ((f_host, "f_host"), (u_host, "u_host")):
+            if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+                    and t.dim() == 4 and tuple(t.shape[1:]) == self.shape and t.shape[0] == f_host.shape[0]):
+                raise ValueError(f"{name}: need a contiguous float64 CPU tensor of shape (nbatch,) + {self.shape}")
+        s = torch.cuda.current_stream() if stream is None else stream
+        st = pp_solve_host_batch(self.handle, f_host.data_ptr(), u_host.data_ptr(), int(f_host.shape[0]), s.cuda_stream)
+        if st != PP_SUCCESS:
+            raise PittPackError(st, "pp_solve_host_batch")
         return u_host
 
     def set_profiling(self, enable: bool):

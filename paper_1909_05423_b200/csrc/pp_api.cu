@@ -32,6 +32,11 @@ struct pp_plan {
     double *sx, *sy;           // dz^2 lam / h^2 per packed position
     double *zero_scratch;      // [nz]
     double *host_stage;        // N doubles, created by the first pp_solve_host
+    // pp_solve_host_batch: a ring of staging buffers, a copy-in and a copy-out stream, events per buffer
+    static constexpr int NSTAGE = 3;
+    double *batch_stage[NSTAGE];
+    cudaStream_t s_in, s_out;
+    cudaEvent_t ev_in[NSTAGE], ev_done[NSTAGE], ev_out[NSTAGE];
     size_t bytes;
     int profiling;
     int have_times;
@@ -349,6 +354,14 @@ void free_plan(pp_plan *p) {
     if (p->ev_fork) cudaEventDestroy(p->ev_fork);
     if (p->ev_join) cudaEventDestroy(p->ev_join);
     if (p->side) cudaStreamDestroy(p->side);
+    for (int b = 0; b < pp_plan::NSTAGE; ++b) {
+        cudaFree(p->batch_stage[b]);
+        if (p->ev_in[b]) cudaEventDestroy(p->ev_in[b]);
+        if (p->ev_done[b]) cudaEventDestroy(p->ev_done[b]);
+        if (p->ev_out[b]) cudaEventDestroy(p->ev_out[b]);
+    }
+    if (p->s_in) cudaStreamDestroy(p->s_in);
+    if (p->s_out) cudaStreamDestroy(p->s_out);
     cudaGetLastError();
     delete p;
 }
@@ -513,6 +526,49 @@ int pp_solve_host(pp_plan *plan, const double *f_host, double *u_host, void *str
     if (int rc = pp_solve(plan, plan->host_stage, plan->host_stage, stream)) return rc;
     if (cudaMemcpyAsync(u_host, plan->host_stage, nb, cudaMemcpyDeviceToHost, st) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
     if (cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    return PP_SUCCESS;
+}
+
+int pp_solve_host_batch(pp_plan *plan, const double *f_host, double *u_host, int nbatch, void *stream) {
+    if (!plan || !f_host || !u_host) return PP_ERR_NULL;
+    if (nbatch < 1) return PP_ERR_INVALID_ARG;
+    const size_t n = (size_t)plan->nx * plan->ny * plan->nz, nb = n * sizeof(double);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int nstage = nbatch < pp_plan::NSTAGE ? nbatch : pp_plan::NSTAGE;
+    // lazily: staging ring, copy streams, events
+    if (!plan->s_in) {
+        if (cudaStreamCreateWithFlags(&plan->s_in, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaStreamCreateWithFlags(&plan->s_out, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    }
+    for (int b = 0; b < nstage; ++b) {
+        if (!plan->batch_stage[b]) {
+            if (cudaMalloc((void **)&plan->batch_stage[b], nb) != cudaSuccess) { plan->batch_stage[b] = nullptr; cudaGetLastError(); return PP_ERR_ALLOC; }
+            plan->bytes += nb;
+        }
+        if (!plan->ev_in[b]) {
+            if (cudaEventCreateWithFlags(&plan->ev_in[b], cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&plan->ev_done[b], cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&plan->ev_out[b], cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+        }
+    }
+#define PP_CK(call) if ((call) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    // copy-in of right-hand side i+1 and copy-out of solution i-1 run beside the solve of i (PCIe is full duplex)
+    for (int i = 0; i < nbatch; ++i) {
+        const int b = i % nstage;
+        double *d = plan->batch_stage[b];
+        if (i >= nstage) PP_CK(cudaStreamWaitEvent(plan->s_in, plan->ev_out[b], 0))          // buffer free again
+        PP_CK(cudaMemcpyAsync(d, f_host + (size_t)i * n, nb, cudaMemcpyHostToDevice, plan->s_in))
+        PP_CK(cudaEventRecord(plan->ev_in[b], plan->s_in))
+        PP_CK(cudaStreamWaitEvent(st, plan->ev_in[b], 0))
+        if (int rc = pp_solve(plan, d, d, stream)) return rc;
+        PP_CK(cudaEventRecord(plan->ev_done[b], st))
+        PP_CK(cudaStreamWaitEvent(plan->s_out, plan->ev_done[b], 0))
+        PP_CK(cudaMemcpyAsync(u_host + (size_t)i * n, d, nb, cudaMemcpyDeviceToHost, plan->s_out))
+        PP_CK(cudaEventRecord(plan->ev_out[b], plan->s_out))
+    }
+    PP_CK(cudaStreamSynchronize(plan->s_out))
+    PP_CK(cudaStreamSynchronize(st))
+#undef PP_CK
     return PP_SUCCESS;
 }
 

@@ -199,3 +199,22 @@ def test_fold_dirichlet_faces_matches_the_oracle():
         plan.fold_dirichlet(ft, {("x", 0): torch.zeros(nz, ny, dtype=torch.float64, device="cuda")})
     plan.fold_dirichlet(ft, {("z", 1): torch.zeros(ny, nx, dtype=torch.float64, device="cuda")})
     plan.destroy()
+
+
+def test_host_batch_pipeline():
+    """pp_solve_host_batch: five right-hand sides through a ring of three staging buffers; every solution
+    equals the one-at-a-time host solve bit for bit."""
+    import torch
+    import paper_1909_05423_b200 as pp
+    w = wl.config2("PPN", "normal", n=64)
+    plan = pp.Plan(64, 64, 64, *w.h, w.bc)
+    fb = torch.stack([torch.from_numpy(wl.random_normal(w.shape, 40 + i, zero_mean=True)) for i in range(5)]).pin_memory()
+    ub = torch.empty_like(fb).pin_memory()
+    plan.solve_host_batch(fb, ub)
+    one = torch.empty(w.shape, dtype=torch.float64).pin_memory()
+    for i in range(5):
+        plan.solve_host(fb[i].contiguous().pin_memory(), one)
+        assert torch.equal(ub[i], one), i
+    assert rel_err(ub[4].numpy(), po.solve(fb[4].numpy(), w.h, w.bc)) <= TOL
+    plan.solve_host_batch(fb[:2], ub[:2])              # shorter than the ring
+    plan.destroy()
