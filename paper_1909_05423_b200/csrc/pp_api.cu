@@ -64,7 +64,7 @@ bool length_supported(int n) { return n >= 4 && n <= 2048 && fft_length_ok(n); }
 void make_twiddles(int n, std::vector<double2> &tw, std::vector<double2> &ptw) {
     tw.assign(tw_table_elems(n), make_double2(1.0, 0.0));
     ptw.resize(n + 1);
-    // stage with NS: rows r = 1, 2, 4 (radix 8) or r = 1, 2 (radix 4) of W_n^(k r stride), stride = n / (RS NS), k in [0, NS)
+    // stage with NS: row r = 1 (radix 8) or rows r = 1, 2 (radix 4) of W_n^(k r stride), stride = n / (RS NS), k in [0, NS)
     const int rs = stage_radix(n), rows = tw_rows(n);
     for (int ns = first_radix(n); ns < n; ns *= rs) {
         const int off = tw_stage_offset(n, ns), stride = n / (rs * ns);

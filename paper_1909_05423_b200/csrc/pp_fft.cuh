@@ -55,9 +55,9 @@ struct FftCfg {
 
 // Stage twiddle tables.  Every stage after the first has radix RS (8 or 4) and multiplies input r of
 // butterfly j by W_N^(k r STRIDE), k = j mod NS, STRIDE = N / (RS NS).  The plan stores, per stage, the
-// rows r = 1, 2, 4 (RS = 8) or r = 1, 2 (RS = 4) as [r][k] -- contiguous in k, so a warp's 16-byte loads
+// row r = 1 (RS = 8) or the rows r = 1, 2 (RS = 4) as [r][k] -- contiguous in k, so a warp's 16-byte loads
 // touch NS*16 contiguous bytes instead of lines STRIDE*16 bytes apart; the other powers are products.
-__host__ __device__ constexpr int tw_rows(int n) { return stage_radix(n) == 8 ? 3 : 2; }
+__host__ __device__ constexpr int tw_rows(int n) { return stage_radix(n) == 8 ? 1 : 2; }
 __host__ __device__ constexpr int tw_stage_offset(int n, int NS) {
     int off = 0;
     for (int ns = first_radix(n); ns < NS; ns *= stage_radix(n)) off += tw_rows(n) * ns;
@@ -222,12 +222,13 @@ __device__ __forceinline__ void fft_stage(double2 (&v)[FftCfg<N>::E], int t, dou
         for (int r = 0; r < R; ++r) x[r] = v[b + B * r];
         const int k = j % NS;
         if constexpr (NS > 1 && R == 8) {
-            // W^(k r STRIDE): load r = 1, 2, 4 from the stage table, build the rest with one product each
+            // W^(k r STRIDE): r = 1 from the stage table, the other six powers by products (two squarings and
+            // four multiplies: the loads cost more than the arithmetic here; relative error of W^7 ~ 1e-15)
             const double2 *ts = tw + tw_stage_offset(N, NS);
             double2 w1 = __ldg(&ts[k]);
-            double2 w2 = __ldg(&ts[NS + k]);
-            double2 w4 = __ldg(&ts[2 * NS + k]);
-            if (DIR == INV) { w1 = cconj(w1); w2 = cconj(w2); w4 = cconj(w4); }
+            if (DIR == INV) w1 = cconj(w1);
+            const double2 w2 = cmul(w1, w1);
+            const double2 w4 = cmul(w2, w2);
             const double2 w3 = cmul(w1, w2);
             x[1] = cmul(x[1], w1);
             x[2] = cmul(x[2], w2);
