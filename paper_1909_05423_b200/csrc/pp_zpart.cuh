@@ -163,7 +163,7 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
     }
     double y[R];
 #pragma unroll
-    for (int i = 0; i < R; ++i) y[i] = __ldcs(row0 + i * step);
+    for (int i = 0; i < R; ++i) y[i] = __ldcg(row0 + i * step);
 
     // While the loads fly: thread 0 of the system tabulates the first block, thread jint the interior
     // block, thread jfac factors the interface matrix.
