@@ -24,7 +24,6 @@
 #pragma once
 #include <cuda_runtime.h>
 
-#include "pp_async.cuh"
 
 namespace pp {
 
