@@ -24,3 +24,11 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+@pytest.fixture(scope="session", autouse=True)
+def built_library():
+    """Build libpittpack_b200.so once per session if it is missing or stale (nvcc cross-compiles without a
+    GPU).  The binding itself never builds: it fails loudly when the library is absent."""
+    from paper_1909_05423_b200 import build
+    return build.build()
