@@ -1,0 +1,46 @@
+"""GPU parity on seeded random configurations: sizes drawn from every supported transform length (powers of
+two, 3*2^k, 5*2^k), nz both partitionable and not, all boundary conditions, anisotropic spacings.  Ground truth is
+the oracle with its z solve in long double; the bar is 1e-11 unless the configuration itself is ill-conditioned
+(smallest non-zero shift |s| tiny: an fp64 elimination then carries eps/|s|, SURVEY.md 8(c) hazards)."""
+import numpy as np
+import pytest
+
+from oracle import poisson_oracle as po
+from paper_1909_05423_b200 import workloads as wl
+from gpu_util import TOL, gpu_solve, rel_err
+
+pytestmark = pytest.mark.gpu
+
+LENGTHS = [4, 8, 16, 32, 64, 128, 48, 96, 192, 80, 160]
+NZ = [2, 3, 7, 16, 31, 32, 33, 64, 96, 100, 128, 160, 200, 256, 288, 320, 512]
+
+
+def draw(seed):
+    rng = np.random.default_rng(7000 + seed)
+    nx, ny = int(rng.choice(LENGTHS)), int(rng.choice(LENGTHS))
+    nz = int(rng.choice(NZ))
+    bc = tuple(int(b) for b in rng.integers(0, 3, size=3))
+    h = tuple(float(v) for v in np.exp(rng.uniform(np.log(0.02), np.log(0.5), size=3)))
+    return nx, ny, nz, bc, h
+
+
+def min_shift(nx, ny, bc, h):
+    """smallest non-zero |s| = dz^2 |lam_x/dx^2 + lam_y/dy^2| over the modes (Table 2)"""
+    def lams(n, b):
+        k = np.arange(n)
+        arg = {0: 2 * np.pi * k / n, 1: np.pi * k / n, 2: np.pi * (k + 1) / n}[b]
+        return -4.0 * np.sin(arg / 2) ** 2
+    s = h[2] ** 2 * np.add.outer(lams(ny, bc[1]) / h[1] ** 2, lams(nx, bc[0]) / h[0] ** 2)
+    s = np.abs(s[np.abs(s) > 0])
+    return float(s.min()) if s.size else 1.0
+
+
+@pytest.mark.parametrize("seed", range(40))
+def test_random_configuration(seed):
+    nx, ny, nz, bc, h = draw(seed)
+    shape = (nz, ny, nx)
+    f = wl.random_normal(shape, 8000 + seed, zero_mean=all(b in (0, 1) for b in bc))
+    ref = po.solve(f, h, bc, zdtype=np.longdouble)
+    tol = max(TOL, 200 * np.finfo(np.float64).eps / min_shift(nx, ny, bc, h)) if bc[2] != 2 else TOL
+    e = rel_err(gpu_solve(f, h, bc), ref)
+    assert e <= tol, (nx, ny, nz, bc, h, e, tol)
