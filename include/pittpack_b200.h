@@ -57,7 +57,8 @@ enum {
     PP_ERR_NULL = 5              /* a required pointer argument is NULL */
 };
 
-/* Number of kernels one pp_solve launches, and their order (for pp_plan_last_kernel_ms). */
+/* The five passes of one pp_solve and their order: the timing slots of pp_plan_last_kernel_ms.  By default each
+ * is one kernel; a slot can hold several (two-level z solve) or none (x+y fusion): pp_plan_launches_per_solve. */
 enum { PP_K_XFWD = 0, PP_K_YFWD = 1, PP_K_ZSOLVE = 2, PP_K_YINV = 3, PP_K_XINV = 4, PP_NUM_KERNELS = 5 };
 
 /*
@@ -113,8 +114,8 @@ int pp_plan_destroy(pp_plan *plan);
 size_t pp_plan_workspace_bytes(const pp_plan *plan);
 
 /*
- * Per-kernel timing for roofline reports.  With profiling enabled, pp_solve brackets each of
- * its PP_NUM_KERNELS launches with CUDA events on the caller's stream (no synchronisation).
+ * Per-pass timing for roofline reports.  With profiling enabled, pp_solve brackets each of
+ * its PP_NUM_KERNELS passes with CUDA events on the caller's stream (no synchronisation).
  * pp_plan_last_kernel_ms synchronises on the last event and writes PP_NUM_KERNELS
  * durations in milliseconds (order PP_K_*) into ms_out (host pointer).
  */
