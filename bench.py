@@ -2,11 +2,15 @@
 """Benchmark of the direct Poisson solve (BASELINE.json metric: Gpoints/s per fp64 Poisson solve and
 % of HBM roofline at 512x512x256).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg3|cfg4|cfg5|cfg2|pencil] [--fusion]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+                    [--workload cfg3|cfg1|cfg2|cfg4|cfg5|pencil|pencil48] [--fusion] [--no-cpu-baseline]
 
 A "step" is one pp_solve: the whole hot path (x-fwd, y-fwd, z-solve, y-inv, x-inv) over one synthetic
 grid.  N > 1 runs N independent replicas (one process per GPU, no data-path collective -- DESIGN.md
-"replicas only"); value = points solved by all ranks / max-over-ranks device time.
+"replicas only"); value = points solved by all ranks / max-over-ranks device time.  `e2e` is the same
+metric through the host-buffer entry point (pp_solve_host_batch: every step's H2D and D2H inside the
+timed region, copies of neighbouring steps pipelined with the solves); `roofline` is the slowest pass
+against the measured HBM copy bandwidth, `roofline_solve` the whole solve against 80 B/point.
 
 Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for the definition of every field.
 """
