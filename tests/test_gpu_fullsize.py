@@ -1,10 +1,11 @@
 """Parity at BASELINE.json's full sizes, in the launch configuration bench.py times.
 
-config 3 (512x512x256, the headline) is small enough for the oracle to solve whole (~15-20 s of
-host time), so it is compared element by element.  configs 4 and 5 (2^30 and 2^29 points) are
-checked on sampled outputs the oracle computes one by one -- the 7-point residual of eq. 3
- at sampled cells, and for the eigenfunction twin the closed-form discrete solution --
-properties that pin the solution of a non-singular linear system at any size."""
+Every configuration is compared with the oracle element by element: config 3 (512x512x256, the headline)
+by ``po.solve`` on the whole array; configs 4 and 5 (2^30 and 2^29 points) by the oracle's own functions
+applied block by block on the host (tests/oracle_blocked.py -- the whole-array temporaries of ``po.solve`` would
+need > 60 GB), a few minutes of host time each.  Kept beside them: the 7-point residual of eq. 3
+ at 300 000 sampled cells (checker pinned on the CPU: tests/test_oracle_stencil.py) and, for the
+eigenfunction twin of config 4, the closed-form discrete solution."""
 import math
 
 import numpy as np
@@ -13,6 +14,8 @@ import pytest
 from oracle import poisson_oracle as po
 from paper_1909_05423_b200 import workloads as wl
 from gpu_util import TOL, rel_err
+from oracle_blocked import oracle_solve_blocked
+from stencil_sampling import gather_torch, neighbour_table, sample_indices
 
 pytestmark = pytest.mark.gpu
 
@@ -37,46 +40,9 @@ def test_config3_full_size_element_by_element():
     assert abs(ug.mean()) <= 1e-13 * np.max(np.abs(ug))          # zero-mean invariant
 
 
-def sample_indices(shape, count, seed):
-    """Random cells plus cells on every face, edge and corner."""
-    rng = np.random.default_rng(seed)
-    nz, ny, nx = shape
-    k = rng.integers(0, nz, count)
-    j = rng.integers(0, ny, count)
-    i = rng.integers(0, nx, count)
-    third = count // 3
-    k[:third] = rng.choice([0, nz - 1], third)
-    j[third // 2: third + third // 2] = rng.choice([0, ny - 1], third)
-    i[third: 2 * third] = rng.choice([0, nx - 1], third)
-    return k, j, i
-
-
-def gather_neighbours(u, idx, bc):
-    """(count, 7) array (u_c, u_xm, u_xp, u_ym, u_yp, u_zm, u_zp) with the ghost rules of the three
-    homogeneous boundary conditions: periodic wrap, Neumann mirror, Dirichlet -u."""
-    import torch
-    k, j, i = (torch.from_numpy(v).cuda() for v in idx)
-    cols = [u[k, j, i]]
-    for axis, (n, b) in enumerate(zip((u.shape[2], u.shape[1], u.shape[0]), bc)):
-        for d in (-1, 1):
-            kk, jj, ii = k.clone(), j.clone(), i.clone()
-            t = (ii, jj, kk)[axis]
-            t += d
-            sign = torch.ones_like(cols[0])
-            out = (t < 0) | (t >= n)
-            if b == 0:
-                t %= n
-            else:
-                t.clamp_(0, n - 1)
-                if b == 2:
-                    sign = torch.where(out, -sign, sign)
-            cols.append(sign * u[kk, jj, ii])
-    return torch.stack(cols, dim=1).cpu().numpy()
-
-
 def residual_check(u, f, h, bc, seed):
     idx = sample_indices(tuple(u.shape), 300_000, seed)
-    nb = gather_neighbours(u, idx, bc)
+    nb = gather_torch(u, neighbour_table(idx, tuple(u.shape), bc))   # ghost rules: NumPy, pinned on the CPU
     Au = po.stencil_at(nb, h)                                    # the oracle, one sampled cell at a time
     fs = f[idx]
     fmax = float(np.max(np.abs(fs)))
@@ -135,7 +101,7 @@ def test_config4_full_size_sampled(twin):
     u = plan.solve(f)
     torch.cuda.synchronize()
     idx = sample_indices((n, n, n), 300_000, seed=4)
-    nb = gather_neighbours(u, idx, bc)
+    nb = gather_torch(u, neighbour_table(idx, (n, n, n), bc))
     k, j, i = (torch.from_numpy(v).cuda() for v in idx)
     fs = f[k, j, i].cpu().numpy()
     Au = po.stencil_at(nb, h)
@@ -152,3 +118,66 @@ def test_config4_full_size_sampled(twin):
     else:
         assert float(np.max(np.abs(nb[:, 0] - u_exact))) <= 5e-6     # second-order accurate, h = 1/1025
     plan.destroy()
+
+
+def host_memory_gib():
+    with open("/proc/meminfo") as fh:
+        for line in fh:
+            if line.startswith("MemAvailable"):
+                return int(line.split()[1]) / 2 ** 20
+    return 0.0
+
+
+def solve_to_host(f_dev, h, bc):
+    """GPU solve through the C ABI (default plan: the launch configuration bench.py times), result on the host."""
+    import torch
+    import paper_1909_05423_b200 as pp
+    nz, ny, nx = f_dev.shape
+    plan = pp.Plan(nx, ny, nz, *h, bc)
+    u = plan.solve(f_dev)
+    torch.cuda.synchronize()
+    ug = u.cpu().numpy()
+    plan.destroy()
+    return ug
+
+
+def test_config5_full_size_element_by_element():
+    """2048 x 2048 x 128 NND, every element against the oracle (block-wise driver: tests/oracle_blocked.py)."""
+    import torch
+    if host_memory_gib() < 14:
+        pytest.skip("needs 14 GiB of host memory for the oracle's arrays")
+    w = wl.config5()
+    f = torch.from_numpy(w.f).cuda()
+    ug = solve_to_host(f, w.h, w.bc)
+    del f
+    torch.cuda.empty_cache()
+    ref = oracle_solve_blocked(w.f, w.h, w.bc)                    # in place: w.f now holds the oracle's u
+    e = rel_err_blocked(ug, ref)
+    assert e <= TOL, e
+
+
+@pytest.mark.parametrize("twin", [False, True])
+def test_config4_full_size_element_by_element(twin):
+    """1024^3 DDD as written in BASELINE.json (h = 1/1025, folded faces) and its h = 1/1024 twin, every
+    element against the oracle; the twin also against the closed-form discrete solution (Table 2)."""
+    import torch
+    if host_memory_gib() < 26:
+        pytest.skip("needs 26 GiB of host memory for the oracle's arrays")
+    n = 1024
+    f, g, hh = config4_on_device(n, twin)
+    bc, h = (2, 2, 2), (hh, hh, hh)
+    fh = f.cpu().numpy()
+    ug = solve_to_host(f, h, bc)
+    del f
+    torch.cuda.empty_cache()
+    ref = oracle_solve_blocked(fh, h, bc)
+    e = rel_err_blocked(ug, ref)
+    assert e <= TOL, e
+    if twin:
+        gs = g.cpu().numpy()
+        lam = 3.0 * (2.0 / hh) ** 2 * math.sin(math.pi * hh / 2.0) ** 2
+        worst = 0.0
+        for k0 in range(0, n, 16):
+            closed = (gs[k0:k0 + 16, None, None] * gs[None, :, None] * gs[None, None, :]) * ((3.0 * math.pi ** 2) / lam)
+            worst = max(worst, float(np.max(np.abs(ug[k0:k0 + 16] - closed))))
+        assert worst <= 1e-11, worst
