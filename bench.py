@@ -3,7 +3,7 @@
 % of HBM roofline at 512x512x256).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
-                    [--workload cfg3|cfg1|cfg2|cfg4|cfg5|pencil|pencil48] [--fusion] [--no-cpu-baseline]
+                    [--workload cfg3|cfg1|cfg2|cfg4|cfg5|pencil|pencil48] [--bc PPN] [--fusion] [--no-cpu-baseline]
 
 A "step" is one pp_solve: the whole hot path (x-fwd, y-fwd, z-solve, y-inv, x-inv) over one synthetic
 grid.  N > 1 runs N independent replicas (one process per GPU, no data-path collective -- DESIGN.md
@@ -34,10 +34,12 @@ BYTES_PER_POINT_KERNEL = 16.0    # one pass
 FALLBACK_HBM_GBS = 6650.0        # /opt/skills/guides/B200_PROFILING.md
 
 
-def workload_by_name(name):
+def workload_by_name(name, bc=None):
     from paper_1909_05423_b200 import workloads as wl
+    if bc and name not in ("cfg3", "pencil", "pencil48"):
+        raise SystemExit("--bc applies to the cfg3 grid and the pencils only")
     if name == "cfg3":
-        return wl.config3()
+        return wl.config3(combo=bc or "PPN")
     if name == "cfg4":
         return wl.config4()
     if name == "cfg5":
@@ -47,9 +49,9 @@ def workload_by_name(name):
     if name == "cfg1":
         return wl.config1("uniform")
     if name == "pencil":
-        return wl.paper_pencil("PPN")
+        return wl.paper_pencil(bc or "PPN")
     if name == "pencil48":
-        return wl.paper_pencil("PPN", nxy=48, nz=8192)
+        return wl.paper_pencil(bc or "PPN", nxy=48, nz=8192)
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -68,30 +70,33 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def committed_traffic(kernel):
-    """dram bytes per launch of `kernel` from the committed ncu --set full summary, or None."""
+def committed_traffic(workload, kernel):
+    """dram bytes per launch of pass `kernel` at `workload` from a committed ncu --set full summary
+    (profiles/dram_traffic.csv: workload,kernel,bytes,source), or None when no capture of that workload
+    and kernel is committed."""
     path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
     try:
         with open(path) as fh:
             for line in fh:
                 t = [s.strip() for s in line.split(",")]
-                if len(t) >= 2 and t[0] == kernel:
-                    return float(t[1])
+                if len(t) >= 3 and t[0] == workload and t[1] == kernel:
+                    return float(t[2])
     except Exception:
         pass
     return None
 
 
 class ClockSampler(threading.Thread):
-    """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
+    """Samples SM clock and throttle reasons of one GPU through NVML (about every millisecond) while the
+    measured regions run; a region is the slice of samples between two mark() calls."""
     REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown",
                0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting"}
 
-    def __init__(self, index, period=0.01):
+    def __init__(self, index, period=0.001):
         super().__init__(daemon=True)
         self.index, self.period = index, period
         self.stop_flag = threading.Event()
-        self.mhz, self.reasons, self.max_mhz, self.ok = [], set(), None, False
+        self.mhz, self.masks, self.max_mhz, self.ok = [], [], None, False
 
     def run(self):
         try:
@@ -99,26 +104,34 @@ class ClockSampler(threading.Thread):
             pynvml.nvmlInit()
             h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
             self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            try:
+                pynvml.nvmlDeviceGetCurrentClocksEventReasons(h)
+                reasons = pynvml.nvmlDeviceGetCurrentClocksEventReasons
+            except Exception:
+                reasons = pynvml.nvmlDeviceGetCurrentClocksThrottleReasons
             self.ok = True
             while not self.stop_flag.is_set():
-                self.mhz.append(int(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)))
-                try:
-                    mask = int(pynvml.nvmlDeviceGetCurrentClocksEventReasons(h))
-                except Exception:
-                    mask = int(pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(h))
-                for bit, name in self.REASONS.items():
-                    if mask & bit:
-                        self.reasons.add(name)
+                mhz = int(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM))
+                mask = int(reasons(h))
+                self.masks.append(mask)
+                self.mhz.append(mhz)                     # appended last: len(mhz) <= len(masks)
                 time.sleep(self.period)
         except Exception as exc:  # pragma: no cover
             self.error = repr(exc)
 
-    def result(self):
-        if not self.ok or not self.mhz:
+    def mark(self):
+        return len(self.mhz)
+
+    def result(self, lo=0, hi=None):
+        mhz = self.mhz[lo:hi]
+        if not self.ok or not mhz:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"], "samples": 0}
-        s = sorted(self.mhz)
-        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
-                "samples": len(s)}
+        mask = 0
+        for m in self.masks[lo:(lo + len(mhz))]:
+            mask |= m
+        s = sorted(mhz)
+        return {"sm_mhz": s[len(s) // 2], "sm_min_mhz": s[0], "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(name for bit, name in self.REASONS.items() if mask & bit), "samples": len(s)}
 
 
 def physical_gpu_index(local_rank):
@@ -184,7 +197,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    w = workload_by_name(args.workload)
+    w = workload_by_name(args.workload, args.bc)
     sample = oracle_sample(w, step_seconds=150.0 / max(1, args.steps + args.warmup))
     for _ in range(args.warmup):
         time_oracle(w, sample)
@@ -232,6 +245,35 @@ def whole_job_gpoints(world: int, npts_per_rank: int, ms_step: float) -> float:
 # ------------------------------------------------------------------------------------------
 # the CUDA arm
 # ------------------------------------------------------------------------------------------
+def sampled_residual(u, f, h, bc, count=200_000, seed=11):
+    """max |A u - f| over `count` random cells of the timed solve's output, relative to max |f| -- eq. 3
+     with the ghost rules of the three boundary conditions, by torch gathers on the device.
+    (bench.py's own check that the timed kernels solved the problem; the oracle is not involved.)"""
+    import torch
+    nz, ny, nx = u.shape
+    g = torch.Generator(device="cpu").manual_seed(seed)
+    idx = [torch.randint(0, n, (count,), generator=g).to(u.device) for n in (nz, ny, nx)]
+    uc = u[idx[0], idx[1], idx[2]]
+    fs = f[idx[0], idx[1], idx[2]]
+    if all(b in (0, 1) for b in bc):
+        fs = fs - f.mean()                              # singular: the solve projects f to zero mean
+    acc = torch.zeros_like(uc)
+    for axis, (n, b, hh) in enumerate(zip((nx, ny, nz), bc, h)):
+        for d in (-1, 1):
+            cell = list(idx)
+            t = cell[2 - axis] + d
+            outside = (t < 0) | (t >= n)
+            if b == 0:
+                t = t % n
+                sign = 1.0
+            else:
+                t = t.clamp(0, n - 1)
+                sign = torch.where(outside, -1.0, 1.0) if b == 2 else 1.0
+            cell[2 - axis] = t
+            acc += (sign * u[cell[0], cell[1], cell[2]] - uc) / (hh * hh)
+    return float((acc - fs).abs().max() / f.abs().max())
+
+
 def run_cuda(args):
     import numpy as np
     import torch
@@ -241,6 +283,9 @@ def run_cuda(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py --gpus {args.gpus} but WORLD_SIZE={world}: launch one rank per GPU "
+                         "(python -m torch.distributed.run --nproc-per-node N bench.py --gpus N ...)")
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
     torch.cuda.set_device(local_rank)
@@ -253,7 +298,7 @@ def run_cuda(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    w = workload_by_name(args.workload)
+    w = workload_by_name(args.workload, args.bc)
     nz, ny, nx = w.shape
     npts = w.n_points
     plan = pp.Plan(nx, ny, nz, *w.h, w.bc)
@@ -274,25 +319,28 @@ def run_cuda(args):
     time.sleep(0.05)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
+    m0 = sampler.mark()
     e0.record(stream)
     for _ in range(args.steps):
         plan.solve(f, u)
     e1.record(stream)
     barrier()
-    sampler.stop_flag.set()
-    sampler.join()
+    m1 = sampler.mark()
     ms_total = max_over_ranks(e0.elapsed_time(e1), "cuda")
     ms_step = ms_total / args.steps
     value = whole_job_gpoints(world, npts, ms_step)
+    residual = sampled_residual(u, f, w.h, w.bc)        # of the last timed solve's output
 
     # ---- per-kernel durations over the same number of steps (CUDA events on the launching stream)
     plan.set_profiling(True)
     sums = dict.fromkeys(pp.KERNEL_NAMES, 0.0)
     barrier()
+    m2 = sampler.mark()
     for _ in range(args.steps):
         plan.solve(f, u)
         for k, v in plan.last_kernel_ms().items():
             sums[k] += v
+    m3 = sampler.mark()
     plan.set_profiling(False)
     kernel_ms = {k: v / args.steps for k, v in sums.items()}
 
@@ -304,6 +352,7 @@ def run_cuda(args):
     uh = torch.empty_like(fh).pin_memory()
     plan.solve_host(fh, uh)
     barrier()
+    m4 = sampler.mark()
     e0.record(stream)
     for _ in range(e2e_steps):
         plan.solve_host(fh, uh)
@@ -323,6 +372,9 @@ def run_cuda(args):
         e2e_api = f"pp_solve_host_batch (pinned host buffers, {nbatch} steps per call, copies pipelined with the solves)"
         e2e_steps = nbatch
         del fb, ub
+    m5 = sampler.mark()
+    sampler.stop_flag.set()
+    sampler.join()
     e2e_value = whole_job_gpoints(world, npts, e2e_ms)
 
     if rank == 0:
@@ -337,6 +389,7 @@ def run_cuda(args):
         dom = max((k for k in kernel_ms if slot_bytes[k] > 0), key=lambda k: kernel_ms[k] / slot_bytes[k])
         achieved = slot_bytes[dom] * npts / (kernel_ms[dom] * 1e-3) / 1e9
         solve_gbs = BYTES_PER_POINT_SOLVE * npts / (ms_step * 1e-3) / 1e9
+        wkey = args.workload + (("-" + args.bc.upper()) if args.bc else "") + ("-fused" if args.fusion else "")
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
@@ -344,32 +397,59 @@ def run_cuda(args):
             "config": {"workload": describe(w), "parallelism": f"replicas x{world} (no collective)",
                        "l2_policy": "inputs larger than L2 (f and u are %d MiB each)" % (npts * 8 >> 20),
                        "in_place": False, "xy_fusion": bool(args.fusion), "kernels_per_solve": launches},
-            "clocks": sampler.result(),
+            "clocks": sampler.result(m0, m1),
+            "clocks_regions": {"per_kernel_timing": sampler.result(m2, m3), "e2e": sampler.result(m4, m5)},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": npts * 8, "d2h_bytes_per_step": npts * 8,
                     "ms_per_step": e2e_ms, "steps": e2e_steps, "api": e2e_api,
                     "single_call": {"value": whole_job_gpoints(world, npts, e2e_single_ms), "ms_per_step": e2e_single_ms,
                                     "api": "pp_solve_host"}},
             "gpu_launches": launches * args.steps,
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": committed_traffic(dom), "peak_source": peak_src,
+                         "frac": achieved / peak, "traffic": committed_traffic(wkey, dom), "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": slot_bytes[dom] * npts},
             "roofline_solve": {"bound": "hbm", "achieved": solve_gbs, "peak": peak, "unit": "GB/s",
                                "frac": solve_gbs / peak, "bytes_per_point": BYTES_PER_POINT_SOLVE,
                                "frac_of_nominal_8TBs": solve_gbs / 8000.0},
             "kernel_ms": kernel_ms,
             "kernel_gbs": {k: slot_bytes[k] * npts / (v * 1e-3) / 1e9 for k, v in kernel_ms.items() if slot_bytes[k] > 0},
+            "check": {"sampled_residual_rel": residual,
+                      "what": "max|A u - f| / max|f| at 200000 random cells of the last timed solve's output (eq. 3)"},
         }
         if world == 1 and not args.no_cpu_baseline:
+            # the oracle on a bounded sample of the workload (its first K z planes), and -- the same sample through
+            # the CUDA path -- the parity error that goes with this timing
             sample = oracle_sample(w, step_seconds=18.0)
-            v, dt = time_oracle(w, sample)
-            out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
+            fs = np.ascontiguousarray(w.f[: sample["nz"]])
+            t0 = time.perf_counter()
+            from oracle import poisson_oracle as po
+            ref = po.solve(fs, w.h, w.bc)
+            dt = time.perf_counter() - t0
+            out["cpu_baseline"] = {"value": fs.size / dt / 1e9, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
                                    "sample": sample["text"], "seconds": dt}
+            if pp.pp_size_supported(nx, ny, sample["nz"], w.bc[2]):
+                p2 = pp.Plan(nx, ny, sample["nz"], *w.h, w.bc)
+                us = p2.solve(torch.from_numpy(fs).cuda()).cpu().numpy()
+                p2.destroy()
+                out["cpu_baseline"]["parity_max_rel_err"] = float(np.max(np.abs(us - ref)) / np.max(np.abs(ref)))
         print(json.dumps(out))
     plan.destroy()
     if distributed:
         dist.barrier()
         dist.destroy_process_group()
     return 0
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without a launcher: start one rank per GPU ourselves (the driver's own
+    multi-GPU command is the same torch.distributed.run line)."""
+    import socket
+    import subprocess
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -379,11 +459,16 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="cfg3", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "pencil", "pencil48"])
+    ap.add_argument("--bc", default=None, help="boundary conditions (x, y, z) of the cfg3 grid or a pencil, e.g. NNN; default PPN")
     ap.add_argument("--fusion", action="store_true", help="plane-wise x+y fusion through L2 (opt-in, DESIGN.md)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    if args.bc is not None and (len(args.bc) != 3 or any(c not in "PNDpnd" for c in args.bc)):
+        raise SystemExit("--bc: three letters out of P, N, D")
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return spawn_ranks(args)
     return run_cuda(args)
 
 

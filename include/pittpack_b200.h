@@ -152,7 +152,7 @@ int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm);
  * tasks of ONE persistent kernel, ordered so that a plane's intermediate spectrum stays in the L2
  * cache between its x and y pass: pp_solve then launches 3 kernels (x+y forward, z solve, y+x
  * inverse) and HBM sees 48 instead of 80 bytes per point.  Results are bit-identical to the
- * unfused path.  Needs nx == ny in {128, 256, 512, 1024}; otherwise PP_ERR_UNSUPPORTED_SIZE and the
+ * unfused path.  Needs nx == ny in {128, 256, 512}; otherwise PP_ERR_UNSUPPORTED_SIZE and the
  * plan is left unchanged.  With fusion on, pp_plan_last_kernel_ms reports the fused kernels' times
  * in the PP_K_XFWD and PP_K_XINV slots and 0 for PP_K_YFWD / PP_K_YINV.
  */
@@ -198,6 +198,52 @@ int pp_size_supported(int nx, int ny, int nz, int bc_z);
  * partition for long lines.  0 for a NULL plan.
  */
 int pp_plan_launches_per_solve(const pp_plan *plan);
+
+/*
+ * ---- Slab decomposition over `world` GPUs (one process per GPU) -------------------------------
+ *
+ * The paper's pencil decomposition and all-to-all on NVLink, re-thought: rank r owns the z-slab of
+ * nz/world planes [r nz/world, (r+1) nz/world) of f and u -- the x and y transforms are local to a slab --
+ * and, for the z solve, the (kx, ky)-pencil of ny/world wavenumber rows ky in [q ny/world, (q+1) ny/world), all kx, all
+ * nz planes (the tridiagonal systems are independent per (kx, ky)).  Pencil layout: [nz][ny/world][nx],
+ * x fastest.  The two re-orientations are FUSED INTO THE y PASSES: the forward y pass stores each spectral row straight
+ * into the pencil block of the rank that owns it, the inverse y pass loads its rows from there -- no pack / unpack
+ * kernel, no staging.  The library never communicates by itself; it is given the addresses:
+ *
+ *   chunk(r -> q) = the nz/world planes of slab r restricted to the rows of pencil q: [nz/world][ny/world][nx] doubles,
+ *   which is a contiguous piece of pencil q (planes r nz/world ...), starting at pencil_q + r * chunk_elems.
+ *
+ *   fwd_dst[q] : where THIS rank's forward pass writes chunk(rank -> q):  peer memory (pencil_q + rank * chunk_elems,
+ *                mapped through CUDA IPC / a peer-enabled pointer), or chunk q of a local send buffer that an
+ *                all-to-all (NCCL) then delivers -- the receive buffer of that all-to-all IS the pencil.
+ *   inv_src[q] : where THIS rank's inverse pass reads chunk(rank <- q) of the solved pencils: peer memory again
+ *                (pencil_q + rank * chunk_elems), or chunk q of the receive buffer of the return all-to-all, whose send
+ *                buffer is the pencil itself.
+ * Bytes crossing NVLink per GPU, per direction and per exchange: 8 N (world-1) / world^2.
+ *
+ * Call order per solve, with a cross-rank barrier on the stream where marked (the caller's job: an NCCL all-reduce,
+ * or the all-to-all itself):
+ *      pp_slab_forward(f_slab)  |barrier / all-to-all|  pp_slab_zsolve(pencil)  |barrier / all-to-all|  pp_slab_inverse(u_slab)
+ *
+ * Needs nz % world == 0, ny % world == 0, nz/world >= 2, world <= 16; sizes otherwise as pp_plan_create.
+ * Singular problems: the (0,0) line lives on rank 0's pencil, which applies the zero-mode fix -- same result as one GPU.
+ */
+typedef struct pp_slab_plan pp_slab_plan;
+int pp_slab_plan_create(pp_slab_plan **out, int world, int rank, int nx, int ny, int nz, double dx, double dy, double dz,
+                        int bc_x, int bc_y, int bc_z);
+int pp_slab_plan_destroy(pp_slab_plan *plan);
+/* doubles in this rank's slab, = doubles in its pencil: nx ny nz / world;  and in one chunk: nx ny nz / world^2 */
+size_t pp_slab_local_elems(const pp_slab_plan *plan);
+size_t pp_slab_chunk_elems(const pp_slab_plan *plan);
+/* fwd_dst, inv_src: HOST arrays of `world` DEVICE addresses (see above), copied into the plan.  May be called again. */
+int pp_slab_set_exchange(pp_slab_plan *plan, double *const *fwd_dst, const double *const *inv_src);
+/* x forward + y forward on the slab.  f_slab: nz/world planes (read only); work_slab: same size, holds the x spectrum
+ * (f_slab == work_slab allowed).  The y pass writes through fwd_dst.  Stream-ordered, no sync. */
+int pp_slab_forward(const pp_slab_plan *plan, const double *f_slab, double *work_slab, void *stream);
+/* every tridiagonal system of this rank's pencil [nz][ny/world][nx], in place. */
+int pp_slab_zsolve(const pp_slab_plan *plan, double *pencil, void *stream);
+/* y inverse (reading through inv_src) + x inverse, result in u_slab (nz/world planes). */
+int pp_slab_inverse(const pp_slab_plan *plan, double *u_slab, void *stream);
 
 /* Static, NUL-terminated description of a status code. */
 const char *pp_strerror(int status);

@@ -8,4 +8,7 @@ from .binding import (  # noqa: F401
     pp_plan_set_profiling, pp_plan_workspace_bytes, pp_solve, pp_solve_host, strerror, version,
 )
 
-__all__ = ["Plan", "PittPackError", "lib", "version", "strerror"]
+from .binding import pp_size_supported  # noqa: F401
+from .slab import SlabPlan, VirtualRanks  # noqa: F401
+
+__all__ = ["Plan", "SlabPlan", "VirtualRanks", "PittPackError", "lib", "version", "strerror"]

@@ -22,6 +22,8 @@ KERNEL_NAMES = ("x_fwd", "y_fwd", "z_solve", "y_inv", "x_inv")
 EXPORTS = (
     "pp_plan_create", "pp_solve", "pp_solve_host", "pp_solve_host_batch", "pp_plan_destroy", "pp_plan_workspace_bytes",
     "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_plan_set_xy_fusion", "pp_plan_launches_per_solve", "pp_size_supported", "pp_plan_set_null_space", "pp_fold_dirichlet", "pp_strerror", "pp_version",
+    "pp_slab_plan_create", "pp_slab_plan_destroy", "pp_slab_local_elems", "pp_slab_chunk_elems", "pp_slab_set_exchange",
+    "pp_slab_forward", "pp_slab_zsolve", "pp_slab_inverse",
 )
 PP_Z_AUTO, PP_Z_SWEEP, PP_Z_PARTITION = 0, 1, 2
 PP_NULL_ZERO_MEAN, PP_NULL_PIN_PLANE0 = 0, 1
@@ -74,6 +76,22 @@ def lib() -> ctypes.CDLL:
     L.pp_plan_set_null_space.restype = i32
     L.pp_fold_dirichlet.argtypes = [vp] * 9
     L.pp_fold_dirichlet.restype = i32
+    L.pp_slab_plan_create.argtypes = [ctypes.POINTER(vp), i32, i32, i32, i32, i32, dbl, dbl, dbl, i32, i32, i32]
+    L.pp_slab_plan_create.restype = i32
+    L.pp_slab_plan_destroy.argtypes = [vp]
+    L.pp_slab_plan_destroy.restype = i32
+    L.pp_slab_local_elems.argtypes = [vp]
+    L.pp_slab_local_elems.restype = ctypes.c_size_t
+    L.pp_slab_chunk_elems.argtypes = [vp]
+    L.pp_slab_chunk_elems.restype = ctypes.c_size_t
+    L.pp_slab_set_exchange.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp)]
+    L.pp_slab_set_exchange.restype = i32
+    L.pp_slab_forward.argtypes = [vp, vp, vp, vp]
+    L.pp_slab_forward.restype = i32
+    L.pp_slab_zsolve.argtypes = [vp, vp, vp]
+    L.pp_slab_zsolve.restype = i32
+    L.pp_slab_inverse.argtypes = [vp, vp, vp]
+    L.pp_slab_inverse.restype = i32
     L.pp_strerror.argtypes = [i32]
     L.pp_strerror.restype = ctypes.c_char_p
     L.pp_version.argtypes = []
@@ -151,6 +169,46 @@ def pp_fold_dirichlet(plan, f_ptr, gx_lo=0, gx_hi=0, gy_lo=0, gy_hi=0, gz_lo=0, 
     return lib().pp_fold_dirichlet(*args)
 
 
+def pp_slab_plan_create(world, rank, nx, ny, nz, dx, dy, dz, bc_x, bc_y, bc_z):
+    """-> (status, handle)"""
+    h = ctypes.c_void_p(0)
+    st = lib().pp_slab_plan_create(ctypes.byref(h), int(world), int(rank), int(nx), int(ny), int(nz), float(dx), float(dy),
+                                   float(dz), int(bc_x), int(bc_y), int(bc_z))
+    return st, (h.value or 0)
+
+
+def pp_slab_plan_destroy(plan):
+    return lib().pp_slab_plan_destroy(ctypes.c_void_p(plan))
+
+
+def pp_slab_local_elems(plan):
+    return int(lib().pp_slab_local_elems(ctypes.c_void_p(plan)))
+
+
+def pp_slab_chunk_elems(plan):
+    return int(lib().pp_slab_chunk_elems(ctypes.c_void_p(plan)))
+
+
+def pp_slab_set_exchange(plan, fwd_dst, inv_src):
+    """fwd_dst, inv_src: sequences of `world` device addresses."""
+    n = len(fwd_dst)
+    a = (ctypes.c_void_p * n)(*[ctypes.c_void_p(int(v)) for v in fwd_dst])
+    b = (ctypes.c_void_p * n)(*[ctypes.c_void_p(int(v)) for v in inv_src])
+    return lib().pp_slab_set_exchange(ctypes.c_void_p(plan), a, b)
+
+
+def pp_slab_forward(plan, f_ptr, work_ptr, stream=0):
+    return lib().pp_slab_forward(ctypes.c_void_p(plan), ctypes.c_void_p(f_ptr), ctypes.c_void_p(work_ptr), ctypes.c_void_p(stream))
+
+
+def pp_slab_zsolve(plan, pencil_ptr, stream=0):
+    return lib().pp_slab_zsolve(ctypes.c_void_p(plan), ctypes.c_void_p(pencil_ptr), ctypes.c_void_p(stream))
+
+
+def pp_slab_inverse(plan, u_ptr, stream=0):
+    return lib().pp_slab_inverse(ctypes.c_void_p(plan), ctypes.c_void_p(u_ptr), ctypes.c_void_p(stream))
+
+
 def strerror(status: int) -> str:
     return lib().pp_strerror(int(status)).decode()
 
@@ -183,12 +241,16 @@ class Plan:
         if st != PP_SUCCESS:
             raise PittPackError(st, "pp_plan_create")
         self.handle = h
+        import torch
+        self.device = torch.cuda.current_device()      # the plan's tables live there (pp_plan_create)
 
     def _check(self, t, name):
         import torch
         if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
                 and tuple(t.shape) == self.shape):
             raise ValueError(f"{name}: need a contiguous float64 CUDA tensor of shape {self.shape}")
+        if t.device.index != self.device:
+            raise ValueError(f"{name}: tensor on cuda:{t.device.index}, plan created on cuda:{self.device}")
 
     def solve(self, f, u=None, stream=None):
         import torch

@@ -1,55 +1,49 @@
 // C ABI of pittpack_b200 (include/pittpack_b200.h): plan construction, table generation and the
 // five-kernel solve.  No cuFFT / cuSPARSE, no CPU fallback.
-#include "../../include/pittpack_b200.h"
 
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
+#include <set>
 #include <vector>
 
-#include "pp_fft.cuh"
-#include "pp_xpass.cuh"
-#include "pp_ypass.cuh"
-#include "pp_zsolve.cuh"
-#include "pp_zpart.cuh"
-#include "pp_fused.cuh"
+#include "pp_plan.h"
+#include "pp_xpass.cuh"      // XCfg: the radix schedule of the x pass (twiddle tables)
+#include "pp_ypass.cuh"      // YCfg, YRows
+#include "pp_zshape.h"       // zpart_shape, zpart_hier_ok, Z_MAX_CK (host-side size rules)
 
 using namespace pp;
 
-struct pp_plan {
-    int nx, ny, nz;
-    double dx, dy, dz;
-    int bcx, bcy, bcz;
-    int device;
-    int num_sms;
-    int singular;
-    double scale;
-    double2 *tw_x, *tw_y;      // per-stage FFT twiddle tables (pp_fft.cuh, tw_stage_offset)
-    double2 *ptw_x, *ptw_y;    // exp(-i pi m / (2n)), m in [0, n]
-    double *sx, *sy;           // dz^2 lam / h^2 per packed position
-    double *zero_scratch;      // [nz]
-    double *host_stage;        // N doubles, created by the first pp_solve_host
-    // pp_solve_host_batch: a ring of staging buffers, a copy-in and a copy-out stream, events per buffer
-    static constexpr int NSTAGE = 3;
-    double *batch_stage[NSTAGE];
-    cudaStream_t s_in, s_out;
-    cudaEvent_t ev_in[NSTAGE], ev_done[NSTAGE], ev_out[NSTAGE];
-    size_t bytes;
-    int profiling;
-    int have_times;
-    int z_algorithm;           // PP_Z_AUTO / PP_Z_SWEEP / PP_Z_PARTITION
-    double bmax;               // largest |diagonal| of any z system, 3 + max |s| (range check of the partitioned kernels)
-    int null_space;            // PP_NULL_ZERO_MEAN / PP_NULL_PIN_PLANE0 (singular problems only)
-    int xy_fusion;             // 1: x and y passes of a plane run as tasks of one kernel (pp_fused.cuh)
-    int *fuse_sync;            // [1 + nz] ticket + per-plane completion counters
-    double *hier_scratch;      // [4][nz / 256][nx ny]: interface values of the two-level z solve (long lines only)
-    cudaStream_t side;         // long singular lines only: the zero-mode line is solved beside the two-level passes
-    cudaEvent_t ev_fork, ev_join;
-    cudaEvent_t ev[PP_NUM_KERNELS + 1];
+namespace pp {
+struct SmemKey {
+    int device; const void *fn; size_t smem;
+    bool operator<(const SmemKey &o) const {
+        if (device != o.device) return device < o.device;
+        if (fn != o.fn) return fn < o.fn;
+        return smem < o.smem;
+    }
 };
+static std::mutex g_smem_mutex;
+static std::set<SmemKey> g_smem_done;
+
+int set_smem_once(const void *kernel, size_t smem) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    const SmemKey key{dev, kernel, smem};
+    std::lock_guard<std::mutex> lock(g_smem_mutex);
+    if (g_smem_done.count(key)) return PP_SUCCESS;
+    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+        cudaGetLastError();
+        return PP_ERR_CUDA;
+    }
+    g_smem_done.insert(key);
+    return PP_SUCCESS;
+}
+}  // namespace pp
 
 // ------------------------------------------------------------------------------------------
 // host-side tables, evaluated in long double and rounded once
@@ -61,17 +55,18 @@ const long double PI_L = 3.14159265358979323846264338327950288L;
 // powers of two in [4, 2048], 3 * 2^k in [48, 1536], 5 * 2^k in [80, 1280]
 bool length_supported(int n) { return n >= 4 && n <= 2048 && fft_length_ok(n); }
 
-void make_twiddles(int n, std::vector<double2> &tw, std::vector<double2> &ptw) {
-    tw.assign(tw_table_elems(n), make_double2(1.0, 0.0));
+// e: elements per thread of the pass that will use the table (fixes the radix schedule, pp_fft.cuh)
+void make_twiddles(int n, int e, std::vector<double2> &tw, std::vector<double2> &ptw) {
+    tw.assign(tw_table_elems(n, e), make_double2(1.0, 0.0));
     ptw.resize(n + 1);
-    // stage with NS: row r = 1 (radix 8) or rows r = 1, 2 (radix 4) of W_n^(k r stride), stride = n / (RS NS), k in [0, NS)
-    const int rs = stage_radix(n), rows = tw_rows(n);
-    for (int ns = first_radix(n); ns < n; ns *= rs) {
-        const int off = tw_stage_offset(n, ns), stride = n / (rs * ns);
+    // stage with NS: row r = 1 (radix 8, 16) or rows r = 1, 2 (radix 4) of W_n^(k r stride), stride = n / (RS NS), k in [0, NS)
+    const int rs = stage_radix(n, e), rows = tw_rows(n, e);
+    for (int ns = first_radix(n, e); ns < n; ns *= rs) {
+        const int off = tw_stage_offset(n, e, ns), stride = n / (rs * ns);
         for (int ri = 0; ri < rows; ++ri)
             for (int k = 0; k < ns; ++k) {
-                const long long e = ((long long)k * (1 << ri) * stride) % n;
-                const long double a = 2.0L * PI_L * (long double)e / (long double)n;
+                const long long ex = ((long long)k * (1 << ri) * stride) % n;
+                const long double a = 2.0L * PI_L * (long double)ex / (long double)n;
                 tw[off + ri * ns + k] = make_double2((double)cosl(a), (double)(-sinl(a)));
             }
     }
@@ -111,94 +106,6 @@ int upload(T **dst, const std::vector<T> &src, size_t &bytes) {
     return PP_SUCCESS;
 }
 
-// ------------------------------------------------------------------------------------------
-// launch helpers
-// ------------------------------------------------------------------------------------------
-template <class K>
-int set_smem(K kernel, size_t smem) {
-    if (smem > 48 * 1024) {
-        if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
-            cudaGetLastError();
-            return PP_ERR_CUDA;
-        }
-    }
-    return PP_SUCCESS;
-}
-
-template <int N>
-int launch_x(bool fwd, const double *in, double *out, long long npairs, int bc, const double2 *tw,
-             const double2 *ptw, cudaStream_t st) {
-    using X = XCfg<N>;
-    const unsigned grid = (unsigned)((npairs + X::T - 1) / X::T);
-    auto kf = xpass_fwd_kernel<N>;
-    auto ki = xpass_inv_kernel<N>;
-    if (int rc = set_smem(fwd ? kf : ki, X::SMEM)) return rc;
-    if (fwd) kf<<<grid, X::THREADS, X::SMEM, st>>>(in, out, npairs, bc, tw, ptw);
-    else     ki<<<grid, X::THREADS, X::SMEM, st>>>(in, out, npairs, bc, tw, ptw);
-    return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
-}
-
-template <int N>
-int launch_y(bool fwd, double *w, int nxh, int nz, int bc, int complex_cols, const double2 *tw,
-             const double2 *ptw, cudaStream_t st) {
-    using Y = YCfg<N>;
-    const dim3 grid((unsigned)((nxh + Y::T - 1) / Y::T), (unsigned)nz);
-    auto kf = ypass_fwd_kernel<N>;
-    auto ki = ypass_inv_kernel<N>;
-    if (int rc = set_smem(fwd ? kf : ki, Y::SMEM)) return rc;
-    if (fwd) kf<<<grid, Y::THREADS, Y::SMEM, st>>>((double2 *)w, nxh, bc, complex_cols, tw, ptw);
-    else     ki<<<grid, Y::THREADS, Y::SMEM, st>>>((double2 *)w, nxh, bc, complex_cols, tw, ptw);
-    return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
-}
-
-#define PP_DISPATCH_N(n, CALL)                       \
-    switch (n) {                                     \
-        case 4:    return CALL(4);                   \
-        case 8:    return CALL(8);                   \
-        case 16:   return CALL(16);                  \
-        case 32:   return CALL(32);                  \
-        case 64:   return CALL(64);                  \
-        case 128:  return CALL(128);                 \
-        case 256:  return CALL(256);                 \
-        case 512:  return CALL(512);                 \
-        case 1024: return CALL(1024);                \
-        case 2048: return CALL(2048);                \
-        case 48:   return CALL(48);                  \
-        case 96:   return CALL(96);                  \
-        case 192:  return CALL(192);                 \
-        case 384:  return CALL(384);                 \
-        case 768:  return CALL(768);                 \
-        case 1536: return CALL(1536);                \
-        case 80:   return CALL(80);                  \
-        case 160:  return CALL(160);                 \
-        case 320:  return CALL(320);                 \
-        case 640:  return CALL(640);                 \
-        case 1280: return CALL(1280);                \
-        default:   return PP_ERR_UNSUPPORTED_SIZE;   \
-    }
-
-int run_x(const pp_plan *p, bool fwd, const double *in, double *out, cudaStream_t st) {
-    const long long npairs = (long long)p->ny * p->nz / 2;
-#define CALL_X(NN) launch_x<NN>(fwd, in, out, npairs, p->bcx, p->tw_x, p->ptw_x, st)
-    PP_DISPATCH_N(p->nx, CALL_X)
-#undef CALL_X
-}
-
-int run_y(const pp_plan *p, bool fwd, double *w, cudaStream_t st) {
-    const int complex_cols = (p->bcx == PP_BC_PERIODIC && p->bcy == PP_BC_PERIODIC) ? 1 : 0;
-#define CALL_Y(NN) launch_y<NN>(fwd, w, p->nx / 2, p->nz, p->bcy, complex_cols, p->tw_y, p->ptw_y, st)
-    PP_DISPATCH_N(p->ny, CALL_Y)
-#undef CALL_Y
-}
-
-// The partitioned z kernels tabulate the leading minors q_0 .. q_R of a segment block, |q_R| <= bmax^R:
-// for grids so anisotropic (dz >> dx) that this could leave the fp64 range they are not used.
-bool zpart_range_ok(const pp_plan *p, int R) { return (double)R * std::log2(p->bmax) < 1000.0; }
-ZPartShape plan_zpart_shape(const pp_plan *p) {
-    const ZPartShape z = zpart_shape(p->nz);
-    return (z.R && zpart_range_ok(p, z.R)) ? z : ZPartShape{0, 0, 0};
-}
-
 // Non-homogeneous Dirichlet face values moved to the right-hand side:
 //   f[offset + i sf + j ss] -= coef g[j nf + i],   coef = 2 / h^2,  (i, j) over one face of nf x ns cells
 __global__ void fold_face_kernel(double *f, const double *__restrict__ g, int nf, int ns, long long sf, long long ss,
@@ -208,142 +115,6 @@ __global__ void fold_face_kernel(double *f, const double *__restrict__ g, int nf
         double *cell = f + offset + i * sf + j * ss;
         *cell = *cell - __dmul_rn(coef, g[(long long)j * nf + i]);      // two roundings, like the oracle (no FMA)
     }
-}
-
-// nx == ny in {128, 256, 512, 1024}: the sizes the fused x+y kernel is instantiated for
-bool fusion_supported(int nx, int ny) { return nx == ny && nx >= 128 && nx <= 1024 && (nx & (nx - 1)) == 0; }
-
-#ifndef PP_FUSE_LAG
-#define PP_FUSE_LAG 0          // 0: derived from the number of resident CTAs
-#endif
-
-template <int N, bool FWD_DIR>
-int launch_fused(const pp_plan *p, const double *in, double *u, cudaStream_t st) {
-    using Y = YCfg<N>;
-    constexpr int TX = Y::THREADS / FftCfg<N>::P;
-    auto kernel = xy_fused_kernel<N, FWD_DIR>;
-    if (int rc = set_smem(kernel, Y::SMEM)) return rc;
-    int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, Y::THREADS, Y::SMEM) != cudaSuccess || per_sm < 1) {
-        cudaGetLastError();
-        return PP_ERR_CUDA;
-    }
-    FusedParams fp;
-    fp.nz = p->nz; fp.nxh = p->nx / 2;
-    fp.pairs_per_plane = p->ny / 2;
-    const int xt = (int)((fp.pairs_per_plane + TX - 1) / TX), yt = (fp.nxh + Y::T - 1) / Y::T;
-    fp.na = FWD_DIR ? xt : yt;
-    fp.nb = FWD_DIR ? yt : xt;
-    const long long resident = (long long)p->num_sms * per_sm;
-    long long lag = PP_FUSE_LAG ? PP_FUSE_LAG : (5 * resident / (4 * (fp.na + fp.nb)) + 2);
-    fp.lag = (int)(lag < 1 ? 1 : (lag > p->nz ? p->nz : lag));
-    fp.bcx = p->bcx; fp.bcy = p->bcy;
-    fp.complex_cols = (p->bcx == PP_BC_PERIODIC && p->bcy == PP_BC_PERIODIC) ? 1 : 0;
-    fp.sync = p->fuse_sync;
-    if (cudaMemsetAsync(p->fuse_sync, 0, sizeof(int) * (size_t)(p->nz + 1), st) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
-    const long long total = (long long)p->nz * (fp.na + fp.nb);
-    const unsigned grid = (unsigned)(total < resident ? total : resident);
-    kernel<<<grid, Y::THREADS, Y::SMEM, st>>>(in, u, fp, p->tw_x, p->ptw_x, p->tw_y, p->ptw_y);
-    return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
-}
-
-int run_fused(const pp_plan *p, bool fwd, const double *in, double *u, cudaStream_t st) {
-    switch (p->nx) {
-        case 128:  return fwd ? launch_fused<128, true>(p, in, u, st) : launch_fused<128, false>(p, in, u, st);
-        case 256:  return fwd ? launch_fused<256, true>(p, in, u, st) : launch_fused<256, false>(p, in, u, st);
-        case 512:  return fwd ? launch_fused<512, true>(p, in, u, st) : launch_fused<512, false>(p, in, u, st);
-        case 1024: return fwd ? launch_fused<1024, true>(p, in, u, st) : launch_fused<1024, false>(p, in, u, st);
-        default:   return PP_ERR_UNSUPPORTED_SIZE;
-    }
-}
-
-int run_z(const pp_plan *p, double *w, cudaStream_t st) {
-    ZParams zp;
-    zp.nx = p->nx; zp.ny = p->ny; zp.nz = p->nz;
-    zp.bcz = p->bcz;
-    zp.singular = p->singular ? (p->null_space == PP_NULL_PIN_PLANE0 ? 2 : 1) : 0;
-    zp.scale = p->scale;
-    zp.sx = p->sx; zp.sy = p->sy;
-    zp.zero_scratch = p->zero_scratch;
-    const size_t plane = (size_t)p->nx * p->ny;
-#ifndef PP_Z_DSMEM
-#define PP_Z_DSMEM 0
-#endif
-#ifndef PP_Z_CB
-#define PP_Z_CB 16
-#endif
-    const bool want_part = p->z_algorithm != PP_Z_SWEEP;
-    const ZPartShape zs = want_part ? plan_zpart_shape(p) : ZPartShape{0, 0, 0};
-    if (zs.R) {
-        // partitioned, register-resident solve: one HBM read + one write per unknown (pp_zpart.cuh)
-        const bool cyc = p->bcz == PP_BC_PERIODIC;
-        const size_t ds = zpart_smem_bytes(zs, cyc);
-        const unsigned grid = (unsigned)((plane + zs.L - 1) / zs.L);
-        const ZHier none = {1, nullptr, nullptr};
-        auto launch = [&](auto kernel) -> int {
-            if (int rc = set_smem(kernel, ds)) return rc;
-            kernel<<<grid, zs.L * zs.S, ds, st>>>(w, zp, zs.S, zs.L, none);
-            return PP_SUCCESS;
-        };
-        int rc;
-        if (zs.R == 32) rc = cyc ? launch(zsolve_part_kernel<32, 0, true>) : launch(zsolve_part_kernel<32, 0, false>);
-        else            rc = cyc ? launch(zsolve_part_kernel<64, 0, true>) : launch(zsolve_part_kernel<64, 0, false>);
-        if (rc) return rc;
-    } else if (want_part && p->hier_scratch) {
-        // long lines: two-level partition, 8 + 16 bytes per unknown (pp_zpart.cuh, ZHier)
-        const ZPartShape hs = {32, ZP_HIER_ROWS / 32, 32};
-        const size_t ds = zpart_smem_bytes(hs);
-        const int nK = p->nz / ZP_HIER_ROWS;
-        const size_t slab = (size_t)nK * plane;
-        const ZHier h = {nK, p->hier_scratch, p->hier_scratch + slab};
-        const dim3 grid((unsigned)((plane + hs.L - 1) / hs.L), (unsigned)nK);
-        if (int rc = set_smem(zsolve_part_kernel<32, 1>, ds)) return rc;
-        if (int rc = set_smem(zsolve_part_kernel<32, 2>, ds)) return rc;
-        if (p->singular) {
-            // the singular (0,0) line touches column 0 only, which the passes below never store and whose
-            // values they discard: it runs beside them on the plan's side stream (fork / join by events)
-            if (cudaEventRecord(p->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(p->side, p->ev_fork, 0) != cudaSuccess) {
-                cudaGetLastError();
-                return PP_ERR_CUDA;
-            }
-            zero_mode_long_kernel<<<1, 1024, 0, p->side>>>(w, plane, p->nz, p->scale, p->null_space == PP_NULL_PIN_PLANE0);
-            if (cudaEventRecord(p->ev_join, p->side) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
-        }
-        zsolve_part_kernel<32, 1><<<grid, hs.L * hs.S, ds, st>>>(w, zp, hs.S, hs.L, h);
-        zsolve_hier_interface_kernel<<<(unsigned)((plane + 63) / 64), 64, 0, st>>>(zp, h, ZP_HIER_ROWS, p->hier_scratch + 2 * slab,
-                                                                             p->hier_scratch + 3 * slab);
-        zsolve_part_kernel<32, 2><<<grid, hs.L * hs.S, ds, st>>>(w, zp, hs.S, hs.L, h);
-        if (p->singular && cudaStreamWaitEvent(st, p->ev_join, 0) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
-    } else if (p->bcz != PP_BC_PERIODIC) {
-        // checkpoint table in shared memory: ceil(nz / CB) x TH doubles per CTA
-#define PP_ZT_LAUNCH(C, T)                                                                           \
-        do {                                                                                         \
-            const size_t ds = (size_t)(((p->nz + 1) / 2 + C - 1) / C) * T * sizeof(double) + PP_Z_DSMEM; \
-            if (int rc = set_smem(zsolve_thomas_kernel<C, T>, ds)) return rc;                        \
-            zsolve_thomas_kernel<C, T><<<(unsigned)((plane + T - 1) / T), T, ds, st>>>(w, zp);       \
-        } while (0)
-#ifdef PP_Z_TH
-        PP_ZT_LAUNCH(PP_Z_CB, PP_Z_TH);
-#else
-        PP_ZT_LAUNCH(PP_Z_CB, 128);
-#endif
-#undef PP_ZT_LAUNCH
-    } else {
-        constexpr int TH = PP_Z_THREADS;
-        const unsigned grid = (unsigned)((plane + TH - 1) / TH);
-        const int cb = (p->nz <= 16 * Z_MAX_CK) ? 16 : ((p->nz <= 32 * Z_MAX_CK) ? 32 : 64);
-        const size_t ds = PP_Z_DSMEM;      // dummy dynamic shared memory: caps resident CTAs per SM
-#define PP_Z_LAUNCH(K, C)                                                                        \
-        do {                                                                                     \
-            if (int rc = set_smem(K<C>, ds)) return rc;                                          \
-            K<C><<<grid, TH, ds, st>>>(w, zp);                                                   \
-        } while (0)
-        if (cb == 16)      PP_Z_LAUNCH(zsolve_cyclic_kernel, 16);
-        else if (cb == 32) PP_Z_LAUNCH(zsolve_cyclic_kernel, 32);
-        else               PP_Z_LAUNCH(zsolve_cyclic_kernel, 64);
-#undef PP_Z_LAUNCH
-    }
-    return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
 }
 
 void free_plan(pp_plan *p) {
@@ -422,10 +193,10 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
     std::vector<double2> tw, ptw;
     std::vector<double> s;
     int rc = PP_SUCCESS;
-    make_twiddles(nx, tw, ptw);
+    make_twiddles(nx, fft_E(nx, PP_X_E16_MIN), tw, ptw);
     if (!rc) rc = upload(&p->tw_x, tw, p->bytes);
     if (!rc) rc = upload(&p->ptw_x, ptw, p->bytes);
-    make_twiddles(ny, tw, ptw);
+    make_twiddles(ny, fft_E(ny, PP_Y_E16_MIN), tw, ptw);
     if (!rc) rc = upload(&p->tw_y, tw, p->bytes);
     if (!rc) rc = upload(&p->ptw_y, ptw, p->bytes);
     const long double dz2 = (long double)dz * (long double)dz;
@@ -438,12 +209,13 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
     if (!rc) rc = upload(&p->sy, s, p->bytes);
     p->bmax = 3.0 - smin;
     // lines beyond the two-sweep kernel's range need the two-level partition (segments of 32 rows)
-    if (!rc && nz > 64 * Z_MAX_CK && !zpart_range_ok(p, 32)) rc = PP_ERR_UNSUPPORTED_SIZE;
+    // (its interface kernel carries the minors over 33 rows before the first renormalisation)
+    if (!rc && nz > 64 * Z_MAX_CK && !zpart_range_ok(p, 33)) rc = PP_ERR_UNSUPPORTED_SIZE;
     if (!rc) {
         std::vector<double> z((size_t)nz, 0.0);
         rc = upload(&p->zero_scratch, z, p->bytes);
     }
-    if (!rc && long_ok && zpart_shape(nz).R == 0 && zpart_range_ok(p, 32)) {
+    if (!rc && long_ok && zpart_shape(nz).R == 0 && zpart_range_ok(p, 33)) {
         const size_t nb = sizeof(double) * 4 * (size_t)(nz / ZP_HIER_ROWS) * (size_t)nx * (size_t)ny;
         if (cudaMalloc((void **)&p->hier_scratch, nb) != cudaSuccess) { p->hier_scratch = nullptr; cudaGetLastError(); rc = PP_ERR_ALLOC; }
         else p->bytes += nb;
@@ -470,8 +242,17 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
     return PP_SUCCESS;
 }
 
+// a plan's tables live on the device that was current at pp_plan_create: every call that launches must
+// find the same device current (a status code instead of an illegal-address fault at the next sync)
+static int check_device(const pp_plan *plan) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    return dev == plan->device ? PP_SUCCESS : PP_ERR_INVALID_ARG;
+}
+
 int pp_solve(const pp_plan *plan, const double *f, double *u, void *stream) {
     if (!plan || !f || !u) return PP_ERR_NULL;
+    if (int rc = check_device(plan)) return rc;
     const size_t n = (size_t)plan->nx * plan->ny * plan->nz;
     if (((uintptr_t)f & 15) || ((uintptr_t)u & 15)) return PP_ERR_INVALID_ARG;
     if (f != u) {
@@ -491,7 +272,7 @@ int pp_solve(const pp_plan *plan, const double *f, double *u, void *stream) {
     } else {
         if ((rc = run_x(plan, true, f, u, st))) return rc;      // a1-a3: x pre / FFT / post
         PP_MARK(1)
-        if ((rc = run_y(plan, true, u, st))) return rc;         // a4-a6: y pre / FFT / post
+        if ((rc = run_y_fwd(plan, u, nullptr, st))) return rc;         // a4-a6: y pre / FFT / post
     }
     PP_MARK(2)
     if ((rc = run_z(plan, u, st))) return rc;                   // a7-a8: diagonal + tridiagonal solve
@@ -500,7 +281,7 @@ int pp_solve(const pp_plan *plan, const double *f, double *u, void *stream) {
         PP_MARK(4)
         if ((rc = run_fused(plan, false, u, u, st))) return rc; // a9-a10 as tasks of one kernel
     } else {
-        if ((rc = run_y(plan, false, u, st))) return rc;        // a9: y inverse
+        if ((rc = run_y_inv(plan, u, nullptr, st))) return rc;        // a9: y inverse
         PP_MARK(4)
         if ((rc = run_x(plan, false, u, u, st))) return rc;     // a10: x inverse
     }
@@ -512,6 +293,7 @@ int pp_solve(const pp_plan *plan, const double *f, double *u, void *stream) {
 
 int pp_solve_host(pp_plan *plan, const double *f_host, double *u_host, void *stream) {
     if (!plan || !f_host || !u_host) return PP_ERR_NULL;
+    if (int rc = check_device(plan)) return rc;
     const size_t nb = (size_t)plan->nx * plan->ny * plan->nz * sizeof(double);
     if (!plan->host_stage) {
         if (cudaMalloc((void **)&plan->host_stage, nb) != cudaSuccess) {
@@ -532,6 +314,7 @@ int pp_solve_host(pp_plan *plan, const double *f_host, double *u_host, void *str
 int pp_solve_host_batch(pp_plan *plan, const double *f_host, double *u_host, int nbatch, void *stream) {
     if (!plan || !f_host || !u_host) return PP_ERR_NULL;
     if (nbatch < 1) return PP_ERR_INVALID_ARG;
+    if (int rc = check_device(plan)) return rc;
     const size_t n = (size_t)plan->nx * plan->ny * plan->nz, nb = n * sizeof(double);
     cudaStream_t st = (cudaStream_t)stream;
     const int nstage = nbatch < pp_plan::NSTAGE ? nbatch : pp_plan::NSTAGE;
@@ -551,7 +334,16 @@ int pp_solve_host_batch(pp_plan *plan, const double *f_host, double *u_host, int
                 cudaEventCreateWithFlags(&plan->ev_out[b], cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
         }
     }
-#define PP_CK(call) if ((call) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    // on an error in mid-batch the copies and solves already enqueued still use the staging ring: wait for
+    // them before returning, so that a later call cannot reuse a buffer that is in flight
+    auto drain = [&](int rc) {
+        cudaStreamSynchronize(plan->s_in);
+        cudaStreamSynchronize(plan->s_out);
+        cudaStreamSynchronize(st);
+        cudaGetLastError();
+        return rc;
+    };
+#define PP_CK(call) if ((call) != cudaSuccess) { cudaGetLastError(); return drain(PP_ERR_CUDA); }
     // copy-in of right-hand side i+1 and copy-out of solution i-1 run beside the solve of i (PCIe is full duplex)
     for (int i = 0; i < nbatch; ++i) {
         const int b = i % nstage;
@@ -560,7 +352,7 @@ int pp_solve_host_batch(pp_plan *plan, const double *f_host, double *u_host, int
         PP_CK(cudaMemcpyAsync(d, f_host + (size_t)i * n, nb, cudaMemcpyHostToDevice, plan->s_in))
         PP_CK(cudaEventRecord(plan->ev_in[b], plan->s_in))
         PP_CK(cudaStreamWaitEvent(st, plan->ev_in[b], 0))
-        if (int rc = pp_solve(plan, d, d, stream)) return rc;
+        if (int rc = pp_solve(plan, d, d, stream)) return drain(rc);
         PP_CK(cudaEventRecord(plan->ev_done[b], st))
         PP_CK(cudaStreamWaitEvent(plan->s_out, plan->ev_done[b], 0))
         PP_CK(cudaMemcpyAsync(u_host + (size_t)i * n, d, nb, cudaMemcpyDeviceToHost, plan->s_out))
@@ -577,6 +369,91 @@ int pp_plan_destroy(pp_plan *plan) {
     return PP_SUCCESS;
 }
 
+// ---- slab decomposition (include/pittpack_b200.h, "Slab decomposition") --------------------------------------
+struct pp_slab_plan {
+    int world, rank;
+    pp_plan *slab;      // nx x ny x nz/world: tables of the x and y passes
+    pp_plan *full;      // nx x ny x nz: z-solve tables (shift tables, scratch); never solved as a whole
+    pp_plan zview;      // `full` seen from this rank's pencil: ny/world rows starting at ky = rank ny/world
+    YRows fwd, inv;
+    int have_exchange;
+};
+
+int pp_slab_plan_create(pp_slab_plan **out, int world, int rank, int nx, int ny, int nz, double dx, double dy, double dz,
+                        int bc_x, int bc_y, int bc_z) {
+    if (!out) return PP_ERR_NULL;
+    *out = nullptr;
+    if (world < 1 || world > PP_MAX_WORLD || rank < 0 || rank >= world) return PP_ERR_INVALID_ARG;
+    if (nz <= 0 || ny <= 0 || nz % world || ny % world || nz / world < 2) return PP_ERR_UNSUPPORTED_SIZE;
+    pp_slab_plan *sp = new (std::nothrow) pp_slab_plan();
+    if (!sp) return PP_ERR_ALLOC;
+    std::memset(sp, 0, sizeof(*sp));
+    sp->world = world; sp->rank = rank;
+    int rc = pp_plan_create(&sp->slab, nx, ny, nz / world, dx, dy, dz, bc_x, bc_y, bc_z);
+    if (!rc) rc = pp_plan_create(&sp->full, nx, ny, nz, dx, dy, dz, bc_x, bc_y, bc_z);
+    if (rc) { free_plan(sp->slab); free_plan(sp->full); delete sp; return rc; }
+    const int nyl = ny / world;
+    sp->zview = *sp->full;                       // shares full's device tables; owns nothing
+    sp->zview.ny = nyl;
+    sp->zview.sy = sp->full->sy + (size_t)rank * nyl;
+    sp->zview.singular = (sp->full->singular && rank == 0) ? 1 : 0;     // the (0,0) mode is element 0 of rank 0's pencil
+    sp->fwd.rpb = sp->inv.rpb = nyl;
+    *out = sp;
+    return PP_SUCCESS;
+}
+
+int pp_slab_plan_destroy(pp_slab_plan *plan) {
+    if (!plan) return PP_SUCCESS;
+    free_plan(plan->slab);
+    free_plan(plan->full);
+    delete plan;
+    return PP_SUCCESS;
+}
+
+size_t pp_slab_local_elems(const pp_slab_plan *plan) {
+    return plan ? (size_t)plan->full->nx * plan->full->ny * plan->full->nz / plan->world : 0;
+}
+size_t pp_slab_chunk_elems(const pp_slab_plan *plan) { return plan ? pp_slab_local_elems(plan) / plan->world : 0; }
+
+int pp_slab_set_exchange(pp_slab_plan *plan, double *const *fwd_dst, const double *const *inv_src) {
+    if (!plan || !fwd_dst || !inv_src) return PP_ERR_NULL;
+    for (int q = 0; q < plan->world; ++q) {
+        if (!fwd_dst[q] || !inv_src[q]) return PP_ERR_NULL;
+        if (((uintptr_t)fwd_dst[q] & 15) || ((uintptr_t)inv_src[q] & 15)) return PP_ERR_INVALID_ARG;
+        plan->fwd.base[q] = (double2 *)fwd_dst[q];
+        plan->inv.base[q] = (double2 *)const_cast<double *>(inv_src[q]);
+    }
+    plan->have_exchange = 1;
+    return PP_SUCCESS;
+}
+
+int pp_slab_forward(const pp_slab_plan *plan, const double *f_slab, double *work_slab, void *stream) {
+    if (!plan || !f_slab || !work_slab) return PP_ERR_NULL;
+    if (!plan->have_exchange) return PP_ERR_INVALID_ARG;
+    if (((uintptr_t)f_slab & 15) || ((uintptr_t)work_slab & 15)) return PP_ERR_INVALID_ARG;
+    if (int rc = check_device(plan->slab)) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (int rc = run_x(plan->slab, true, f_slab, work_slab, st)) return rc;       // a1-a3 on the slab
+    return run_y_fwd(plan->slab, work_slab, &plan->fwd, st);                // a4-a6, rows stored to their owners
+}
+
+int pp_slab_zsolve(const pp_slab_plan *plan, double *pencil, void *stream) {
+    if (!plan || !pencil) return PP_ERR_NULL;
+    if ((uintptr_t)pencil & 15) return PP_ERR_INVALID_ARG;
+    if (int rc = check_device(plan->full)) return rc;
+    return run_z(&plan->zview, pencil, (cudaStream_t)stream);                     // a7-a8 on nx * ny/world systems
+}
+
+int pp_slab_inverse(const pp_slab_plan *plan, double *u_slab, void *stream) {
+    if (!plan || !u_slab) return PP_ERR_NULL;
+    if (!plan->have_exchange) return PP_ERR_INVALID_ARG;
+    if ((uintptr_t)u_slab & 15) return PP_ERR_INVALID_ARG;
+    if (int rc = check_device(plan->slab)) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (int rc = run_y_inv(plan->slab, u_slab, &plan->inv, st)) return rc; // a9, rows loaded from their owners
+    return run_x(plan->slab, false, u_slab, u_slab, st);                          // a10
+}
+
 size_t pp_plan_workspace_bytes(const pp_plan *plan) { return plan ? plan->bytes : 0; }
 
 int pp_plan_set_profiling(pp_plan *plan, int enable) {
@@ -589,7 +466,7 @@ int pp_plan_set_profiling(pp_plan *plan, int enable) {
 int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm) {
     if (!plan) return PP_ERR_NULL;
     if (algorithm != PP_Z_AUTO && algorithm != PP_Z_SWEEP && algorithm != PP_Z_PARTITION) return PP_ERR_INVALID_ARG;
-    if (algorithm == PP_Z_PARTITION && plan_zpart_shape(plan).R == 0 && !plan->hier_scratch)
+    if (algorithm == PP_Z_PARTITION && !zpart_single_level(plan) && !plan->hier_scratch)
         return PP_ERR_UNSUPPORTED_SIZE;
     if (algorithm == PP_Z_SWEEP && plan->nz > 64 * Z_MAX_CK) return PP_ERR_UNSUPPORTED_SIZE;
     plan->z_algorithm = algorithm;
@@ -606,6 +483,7 @@ int pp_plan_set_xy_fusion(pp_plan *plan, int enable) {
 int pp_fold_dirichlet(const pp_plan *plan, double *f, const double *gx_lo, const double *gx_hi, const double *gy_lo,
                       const double *gy_hi, const double *gz_lo, const double *gz_hi, void *stream) {
     if (!plan || !f) return PP_ERR_NULL;
+    if (int rc = check_device(plan)) return rc;
     if (((gx_lo || gx_hi) && plan->bcx != PP_BC_DIRICHLET) || ((gy_lo || gy_hi) && plan->bcy != PP_BC_DIRICHLET) ||
         ((gz_lo || gz_hi) && plan->bcz != PP_BC_DIRICHLET))
         return PP_ERR_INVALID_ARG;
@@ -643,7 +521,7 @@ int pp_plan_launches_per_solve(const pp_plan *plan) {
     const bool fused = plan->xy_fusion && fusion_supported(plan->nx, plan->ny);
     int n = fused ? 2 : 4;                                        // x/y passes
     const bool want_part = plan->z_algorithm != PP_Z_SWEEP;
-    if (want_part && plan_zpart_shape(plan).R == 0 && plan->hier_scratch) n += 3 + (plan->singular ? 1 : 0);
+    if (want_part && !zpart_single_level(plan) && plan->hier_scratch) n += 3 + (plan->singular ? 1 : 0);
     else n += 1;
     return n;
 }

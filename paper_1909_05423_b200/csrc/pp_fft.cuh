@@ -1,13 +1,15 @@
 // Complex FFT core shared by the x- and y-pass kernels: a register + shared-memory Stockham
 // autosort FFT, fp64.  Powers of two: radix 8 (leading radix 2 or 4 when log2 N is not a multiple
-// of 3).  3 * 2^k and 5 * 2^k: a leading prime-factor butterfly of 6 / 12 / 10 / 20 points, then radix 4.
+// of 3), or -- long transforms, 16 elements per thread -- radix 16 (leading radix 2, 4 or 8): one
+// shared-memory exchange fewer at N = 1024 and 2048, where the exchanges are what the pass costs.
+// 3 * 2^k and 5 * 2^k: a leading prime-factor butterfly of 6 / 12 / 10 / 20 points, then radix 4.
 //
 // "PittPack performs complex FFT transform for all the transformations": every
 // periodic / Neumann / Dirichlet transform of the solver is this core plus a fused pre- and
 // post-processing step.  The paper calls cuFFT here; this is the hand-written
 // replacement.
 //
-// Thread mapping.  An N-point transform is done by P = N/E threads, E elements per thread (8 for
+// Thread mapping.  An N-point transform is done by P = N/E threads, E elements per thread (8 or 16 for
 // powers of two, 12 or 20 otherwise).  Thread t holds, before and after every stage and on exit, the
 // elements with index t + m*P (m = 0..E-1) in natural order -- so global loads and stores of
 // consecutive threads are contiguous, and the last stage needs no shared-memory round trip.  A stage
@@ -26,44 +28,55 @@ __host__ __device__ constexpr int ilog2(int n) { return n <= 1 ? 0 : 1 + ilog2(n
 
 // Supported lengths: N = odd * 2^k with odd in {1, 3, 5} -- the powers of two of BASELINE.json's grids
 // and the 48- and 80-multiples of the paper's weak-scaling runs.
-//   odd = 1: E = 8 elements per thread, radix-8 stages after a first stage of radix 2, 4 or 8
+//   odd = 1: E = 8 elements per thread, radix-8 stages after a first stage of radix 2, 4 or 8; or
+//            E = 16, radix-16 stages after a first stage of radix 2, 4, 8 or 16 (chosen per pass: fft_E)
 //   odd = 3: E = 12, radix-4 stages after a first stage of radix 12 (k even) or 6 (k odd)
 //   odd = 5: E = 20, radix-4 stages after a first stage of radix 20 (k even) or 10 (k odd)
 // The first stage has no twiddles; its composite butterflies (6, 10, 12, 20) are prime-factor
 // (Good-Thomas) combinations of a 3- or 5-point and a 2- or 4-point DFT, so they need none inside either.
+// Every helper below takes the length n and the elements per thread e of the schedule.
 __host__ __device__ constexpr int fft_odd_part(int n) { return (n % 2 == 0) ? fft_odd_part(n / 2) : n; }
 __host__ __device__ constexpr int fft_log2_part(int n) { return ilog2(n / fft_odd_part(n)); }
 __host__ __device__ constexpr bool fft_length_ok(int n) {
     return n >= 4 && (fft_odd_part(n) == 1 || ((fft_odd_part(n) == 3 || fft_odd_part(n) == 5) && fft_log2_part(n) >= 4));
 }
-__host__ __device__ constexpr int stage_radix(int n) { return fft_odd_part(n) == 1 ? 8 : 4; }   // every stage after the first
-__host__ __device__ constexpr int first_radix(int n) {
-    return fft_odd_part(n) == 1 ? ((ilog2(n) % 3 == 0) ? 8 : ((ilog2(n) % 3 == 1) ? 2 : 4))
-                                : fft_odd_part(n) * ((fft_log2_part(n) % 2 == 0) ? 4 : 2);
+// elements per thread: powers of two from `e16_min` on take 16, shorter ones 8
+__host__ __device__ constexpr int fft_E(int n, int e16_min) {
+    return fft_odd_part(n) == 1 ? ((n >= e16_min && n >= 32) ? 16 : (n >= 8 ? 8 : n)) : 4 * fft_odd_part(n);
+}
+__host__ __device__ constexpr int stage_radix(int n, int e) { return fft_odd_part(n) == 1 ? (e == 16 ? 16 : 8) : 4; }   // every stage after the first
+__host__ __device__ constexpr int first_radix(int n, int e) {
+    return fft_odd_part(n) != 1 ? fft_odd_part(n) * ((fft_log2_part(n) % 2 == 0) ? 4 : 2)
+         : e == 16 ? ((ilog2(n) % 4 == 0) ? 16 : (1 << (ilog2(n) % 4)))
+                   : ((ilog2(n) % 3 == 0) ? 8 : ((ilog2(n) % 3 == 1) ? 2 : 4));
 }
 
-template <int N>
+#ifndef PP_E16_MIN
+#define PP_E16_MIN 1024       // default schedule: 16 elements per thread from this length on
+#endif
+
+template <int N, int E_ = fft_E(N, PP_E16_MIN)>
 struct FftCfg {
     static_assert(fft_length_ok(N), "N = 2^k >= 4, or 3 * 2^k / 5 * 2^k with k >= 4");
     static constexpr int ODD = fft_odd_part(N);
-    static constexpr int E = (ODD == 1) ? (N >= 8 ? 8 : N) : 4 * ODD;   // elements per thread
+    static constexpr int E = E_;                   // elements per thread
     static constexpr int P = N / E;                // threads per transform
-    static constexpr int RS = stage_radix(N);      // radix of every stage after the first
-    static constexpr int R0 = first_radix(N);      // first radix
+    static constexpr int RS = stage_radix(N, E);   // radix of every stage after the first
+    static constexpr int R0 = first_radix(N, E);   // first radix
     static constexpr int SMEM_ELEMS = N + N / 8;   // double2 elements per transform incl. padding
 };
 
-// Stage twiddle tables.  Every stage after the first has radix RS (8 or 4) and multiplies input r of
+// Stage twiddle tables.  Every stage after the first has radix RS (16, 8 or 4) and multiplies input r of
 // butterfly j by W_N^(k r STRIDE), k = j mod NS, STRIDE = N / (RS NS).  The plan stores, per stage, the
-// row r = 1 (RS = 8) or the rows r = 1, 2 (RS = 4) as [r][k] -- contiguous in k, so a warp's 16-byte loads
+// row r = 1 (RS = 8, 16) or the rows r = 1, 2 (RS = 4) as [r][k] -- contiguous in k, so a warp's 16-byte loads
 // touch NS*16 contiguous bytes instead of lines STRIDE*16 bytes apart; the other powers are products.
-__host__ __device__ constexpr int tw_rows(int n) { return stage_radix(n) == 8 ? 1 : 2; }
-__host__ __device__ constexpr int tw_stage_offset(int n, int NS) {
+__host__ __device__ constexpr int tw_rows(int n, int e) { return stage_radix(n, e) == 4 ? 2 : 1; }
+__host__ __device__ constexpr int tw_stage_offset(int n, int e, int NS) {
     int off = 0;
-    for (int ns = first_radix(n); ns < NS; ns *= stage_radix(n)) off += tw_rows(n) * ns;
+    for (int ns = first_radix(n, e); ns < NS; ns *= stage_radix(n, e)) off += tw_rows(n, e) * ns;
     return off;
 }
-__host__ __device__ constexpr int tw_table_elems(int n) { return tw_stage_offset(n, n) > 0 ? tw_stage_offset(n, n) : 1; }
+__host__ __device__ constexpr int tw_table_elems(int n, int e) { return tw_stage_offset(n, e, n) > 0 ? tw_stage_offset(n, e, n) : 1; }
 
 // (N - m) mod N for 0 <= m < N
 template <int N>
@@ -125,6 +138,35 @@ __device__ __forceinline__ void bfly8(double2 (&x)[8]) {
     x[1] = cadd(e1, o1); x[5] = csub(e1, o1);
     x[2] = cadd(e2, o2); x[6] = csub(e2, o2);
     x[3] = cadd(e3, o3); x[7] = csub(e3, o3);
+}
+
+// multiply by the constant (cr + i DIR ci): the forward twiddle (cr, -ci) or its conjugate
+template <int DIR>
+__device__ __forceinline__ double2 cmul_const(double2 a, double cr, double ci) {
+    const double si = (DIR == FWD) ? -ci : ci;
+    return make_double2(fma(a.x, cr, -(a.y * si)), fma(a.x, si, a.y * cr));
+}
+
+// in-place 16-point DFT, 16 = 4 x 4: 4-point DFTs over n1 (n = 4 n1 + n0), twiddles W_16^(n0 k1), 4-point DFTs
+// over n0.  The result is left transposed: X_{k1 + 4 k2} sits in x[4 k1 + k2] -- read it through bfly16_at.
+__host__ __device__ constexpr int bfly16_at(int k) { return 4 * (k & 3) + (k >> 2); }
+template <int DIR>
+__device__ __forceinline__ void bfly16(double2 (&x)[16]) {
+    constexpr double C = 0.92387953251128675613, S = 0.38268343236508977173, H = 0.70710678118654752440;
+#pragma unroll
+    for (int n0 = 0; n0 < 4; ++n0) bfly4<DIR>(x[n0], x[n0 + 4], x[n0 + 8], x[n0 + 12]);   // -> x[n0 + 4 k1]
+    // W_16^(n0 k1) = cos(2 pi m / 16) + i DIR sin(2 pi m / 16), m = n0 k1 in {1, 2, 3, 2, 4, 6, 3, 6, 9}
+    x[1 + 4] = cmul_const<DIR>(x[1 + 4], C, S);
+    x[2 + 4] = cmul_const<DIR>(x[2 + 4], H, H);
+    x[3 + 4] = cmul_const<DIR>(x[3 + 4], S, C);
+    x[1 + 8] = cmul_const<DIR>(x[1 + 8], H, H);
+    x[2 + 8] = rot90<DIR>(x[2 + 8]);
+    x[3 + 8] = cmul_const<DIR>(x[3 + 8], -H, H);
+    x[1 + 12] = cmul_const<DIR>(x[1 + 12], S, C);
+    x[2 + 12] = cmul_const<DIR>(x[2 + 12], -H, H);
+    x[3 + 12] = cmul_const<DIR>(x[3 + 12], -C, -S);
+#pragma unroll
+    for (int k1 = 0; k1 < 4; ++k1) bfly4<DIR>(x[4 * k1], x[4 * k1 + 1], x[4 * k1 + 2], x[4 * k1 + 3]);   // -> x[4 k1 + k2]
 }
 
 // in-place natural-order 3-point DFT
@@ -192,11 +234,16 @@ __device__ __forceinline__ void bfly_pfa(double2 (&x)[A * B]) {
     }
 }
 
+// where output r of bfly<R> is found
+template <int R>
+__host__ __device__ constexpr int bfly_at(int r) { return R == 16 ? bfly16_at(r) : r; }
+
 template <int R, int DIR>
 __device__ __forceinline__ void bfly(double2 (&x)[R]) {
     if constexpr (R == 2) bfly2<DIR>(x[0], x[1]);
     else if constexpr (R == 4) bfly4<DIR>(x[0], x[1], x[2], x[3]);
     else if constexpr (R == 8) bfly8<DIR>(x);
+    else if constexpr (R == 16) bfly16<DIR>(x);
     else if constexpr (R == 6) bfly_pfa<3, 2, DIR>(x);
     else if constexpr (R == 12) bfly_pfa<3, 4, DIR>(x);
     else if constexpr (R == 10) bfly_pfa<5, 2, DIR>(x);
@@ -208,11 +255,11 @@ __device__ __forceinline__ void bfly(double2 (&x)[R]) {
 //     inputs  data[j + r N/R] * W_N^(k r N/(NS R)),  r = 0..R-1
 //     outputs out[(j / NS) NS R + k + q NS],          q = 0..R-1
 // Thread t does the E/R butterflies j = t + b P; their inputs are exactly its elements t + m P.
-template <int N, int R, int NS, int DIR, class Layout, class Sync>
-__device__ __forceinline__ void fft_stage(double2 (&v)[FftCfg<N>::E], int t, double2 *s,
+template <int N, int E, int R, int NS, int DIR, class Layout, class Sync>
+__device__ __forceinline__ void fft_stage(double2 (&v)[E], int t, double2 *s,
                                           const double2 *__restrict__ tw, const Layout &lay, const Sync &sync) {
-    using C = FftCfg<N>;
-    constexpr int E = C::E, P = C::P, B = E / R;
+    using C = FftCfg<N, E>;
+    constexpr int P = C::P, B = E / R;
     constexpr bool LAST = (NS * R == N);
 #pragma unroll
     for (int b = 0; b < B; ++b) {
@@ -221,10 +268,25 @@ __device__ __forceinline__ void fft_stage(double2 (&v)[FftCfg<N>::E], int t, dou
 #pragma unroll
         for (int r = 0; r < R; ++r) x[r] = v[b + B * r];
         const int k = j % NS;
-        if constexpr (NS > 1 && R == 8) {
+        if constexpr (NS > 1 && R == 16) {
+            // W^(k r STRIDE), r = 1..15, from the table's r = 1 by products (depth 4: relative error ~ 1e-15);
+            // every power is used as soon as it exists, so few of them are live at a time
+            const double2 *ts = tw + tw_stage_offset(N, E, NS);
+            double2 w1 = __ldg(&ts[k]);
+            if (DIR == INV) w1 = cconj(w1);
+            const double2 w2 = cmul(w1, w1), w4 = cmul(w2, w2), w8 = cmul(w4, w4);
+            const double2 w3 = cmul(w1, w2);
+            x[1] = cmul(x[1], w1);   x[2] = cmul(x[2], w2);   x[3] = cmul(x[3], w3);   x[4] = cmul(x[4], w4);
+            x[8] = cmul(x[8], w8);
+            x[9] = cmul(x[9], cmul(w8, w1));   x[10] = cmul(x[10], cmul(w8, w2));   x[11] = cmul(x[11], cmul(w8, w3));
+            const double2 w12 = cmul(w8, w4);
+            x[12] = cmul(x[12], w12);
+            x[13] = cmul(x[13], cmul(w12, w1));   x[14] = cmul(x[14], cmul(w12, w2));   x[15] = cmul(x[15], cmul(w12, w3));
+            x[5] = cmul(x[5], cmul(w4, w1));   x[6] = cmul(x[6], cmul(w4, w2));   x[7] = cmul(x[7], cmul(w4, w3));
+        } else if constexpr (NS > 1 && R == 8) {
             // W^(k r STRIDE): r = 1 from the stage table, the other six powers by products (two squarings and
             // four multiplies: the loads cost more than the arithmetic here; relative error of W^7 ~ 1e-15)
-            const double2 *ts = tw + tw_stage_offset(N, NS);
+            const double2 *ts = tw + tw_stage_offset(N, E, NS);
             double2 w1 = __ldg(&ts[k]);
             if (DIR == INV) w1 = cconj(w1);
             const double2 w2 = cmul(w1, w1);
@@ -238,8 +300,8 @@ __device__ __forceinline__ void fft_stage(double2 (&v)[FftCfg<N>::E], int t, dou
             x[6] = cmul(x[6], cmul(w2, w4));
             x[7] = cmul(x[7], cmul(w3, w4));
         } else if constexpr (NS > 1) {
-            static_assert(R == 4, "stages after the first are radix 8 (powers of two) or radix 4 (3 * 2^k, 5 * 2^k)");
-            const double2 *ts = tw + tw_stage_offset(N, NS);
+            static_assert(R == 4, "stages after the first are radix 16 / 8 (powers of two) or radix 4 (3 * 2^k, 5 * 2^k)");
+            const double2 *ts = tw + tw_stage_offset(N, E, NS);
             double2 w1 = __ldg(&ts[k]);
             double2 w2 = __ldg(&ts[NS + k]);
             if (DIR == INV) { w1 = cconj(w1); w2 = cconj(w2); }
@@ -250,11 +312,11 @@ __device__ __forceinline__ void fft_stage(double2 (&v)[FftCfg<N>::E], int t, dou
         bfly<R, DIR>(x);
         if constexpr (LAST) {
 #pragma unroll
-            for (int r = 0; r < R; ++r) v[b + B * r] = x[r];
+            for (int r = 0; r < R; ++r) v[b + B * r] = x[bfly_at<R>(r)];
         } else {
             const int j0 = ((j - k) * R) + k;      // (j / NS) * NS * R + k
 #pragma unroll
-            for (int r = 0; r < R; ++r) s[lay(j0 + r * NS)] = x[r];
+            for (int r = 0; r < R; ++r) s[lay(j0 + r * NS)] = x[bfly_at<R>(r)];
         }
     }
     if constexpr (!LAST) {
@@ -265,22 +327,22 @@ __device__ __forceinline__ void fft_stage(double2 (&v)[FftCfg<N>::E], int t, dou
     }
 }
 
-template <int N, int NS, int DIR, class Layout, class Sync>
-__device__ __forceinline__ void fft_stages(double2 (&v)[FftCfg<N>::E], int t, double2 *s,
+template <int N, int E, int NS, int DIR, class Layout, class Sync>
+__device__ __forceinline__ void fft_stages(double2 (&v)[E], int t, double2 *s,
                                            const double2 *__restrict__ tw, const Layout &lay, const Sync &sync) {
-    constexpr int R = (NS == 1) ? FftCfg<N>::R0 : FftCfg<N>::RS;
-    fft_stage<N, R, NS, DIR>(v, t, s, tw, lay, sync);
-    if constexpr (NS * R < N) fft_stages<N, NS * R, DIR>(v, t, s, tw, lay, sync);
+    constexpr int R = (NS == 1) ? FftCfg<N, E>::R0 : FftCfg<N, E>::RS;
+    fft_stage<N, E, R, NS, DIR>(v, t, s, tw, lay, sync);
+    if constexpr (NS * R < N) fft_stages<N, E, NS * R, DIR>(v, t, s, tw, lay, sync);
 }
 
-// N-point complex DFT (sign DIR, unnormalised).  On entry and exit thread t (0 <= t < P) holds
-// elements t + m P in v[m].  `s` is the transform's shared-memory scratch addressed through `lay`;
-// `sync` synchronises the P threads of this transform.  On exit the scratch is free for reuse
-// (the last exchange ends with a sync).
-template <int N, int DIR, class Layout, class Sync>
-__device__ __forceinline__ void fft(double2 (&v)[FftCfg<N>::E], int t, double2 *s,
+// N-point complex DFT (sign DIR, unnormalised), E elements per thread (deduced from v).  On entry and exit
+// thread t (0 <= t < P = N / E) holds elements t + m P in v[m].  `s` is the transform's shared-memory scratch
+// addressed through `lay`; `sync` synchronises the P threads of this transform.  On exit the scratch is free
+// for reuse (the last exchange ends with a sync).
+template <int N, int DIR, int E, class Layout, class Sync>
+__device__ __forceinline__ void fft(double2 (&v)[E], int t, double2 *s,
                                     const double2 *__restrict__ tw, const Layout &lay, const Sync &sync) {
-    fft_stages<N, 1, DIR>(v, t, s, tw, lay, sync);
+    fft_stages<N, E, 1, DIR>(v, t, s, tw, lay, sync);
 }
 
 }  // namespace pp

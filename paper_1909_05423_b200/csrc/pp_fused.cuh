@@ -92,7 +92,7 @@ xy_fused_kernel(const double *in, double *u, FusedParams p,
                 const double2 *__restrict__ tw_x, const double2 *__restrict__ ptw_x,
                 const double2 *__restrict__ tw_y, const double2 *__restrict__ ptw_y) {
     using Y = YCfg<N>;
-    constexpr int TX = Y::THREADS / FftCfg<N>::P;      // row pairs per x tile (= Y::T)
+    constexpr int TX = Y::THREADS / Y::P;               // row pairs per x tile (= Y::T)
     extern __shared__ double2 smem[];
     __shared__ int s_ticket;
     int *ticket = p.sync, *done = p.sync + 1;

@@ -1,0 +1,28 @@
+// x-pass launchers (a1-a3, a10): one instantiation per supported transform length.
+#include "pp_plan.h"
+#include "pp_xpass.cuh"
+
+namespace pp {
+
+template <int N>
+int launch_x(bool fwd, const double *in, double *out, long long npairs, int bc, const double2 *tw,
+             const double2 *ptw, cudaStream_t st) {
+    using X = XCfg<N>;
+    const unsigned grid = (unsigned)((npairs + X::T - 1) / X::T);
+    auto kf = xpass_fwd_kernel<N>;
+    auto ki = xpass_inv_kernel<N>;
+    if (int rc = set_smem(fwd ? kf : ki, X::SMEM)) return rc;
+    if (fwd) kf<<<grid, X::THREADS, X::SMEM, st>>>(in, out, npairs, bc, tw, ptw);
+    else     ki<<<grid, X::THREADS, X::SMEM, st>>>(in, out, npairs, bc, tw, ptw);
+    return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
+}
+
+int run_x(const pp_plan *p, bool fwd, const double *in, double *out, cudaStream_t st) {
+    const long long npairs = (long long)p->ny * p->nz / 2;
+#define CALL_X(NN) launch_x<NN>(fwd, in, out, npairs, p->bcx, p->tw_x, p->ptw_x, st)
+    PP_DISPATCH_N(p->nx, CALL_X)
+#undef CALL_X
+}
+
+
+}  // namespace pp

@@ -1,0 +1,32 @@
+// y-pass launchers, inverse (a9): one instantiation per supported transform length, in place and
+// (slab decomposition) with rows loaded from their owner ranks' pencil blocks.
+#include "pp_plan.h"
+#include "pp_ypass.cuh"
+
+namespace pp {
+
+template <int N>
+int launch_y_inv(double *w, int nxh, int nz, int bc, int complex_cols, const double2 *tw, const double2 *ptw,
+                 const YRows *rows, cudaStream_t st) {
+    using Y = YCfg<N>;
+    const dim3 grid((unsigned)((nxh + Y::T - 1) / Y::T), (unsigned)nz);
+    if (rows) {
+        auto k = ypass_inv_slab_kernel<N>;
+        if (int rc = set_smem(k, Y::SMEM)) return rc;
+        k<<<grid, Y::THREADS, Y::SMEM, st>>>((double2 *)w, nxh, bc, complex_cols, tw, ptw, *rows);
+    } else {
+        auto k = ypass_inv_kernel<N>;
+        if (int rc = set_smem(k, Y::SMEM)) return rc;
+        k<<<grid, Y::THREADS, Y::SMEM, st>>>((double2 *)w, nxh, bc, complex_cols, tw, ptw);
+    }
+    return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
+}
+
+int run_y_inv(const pp_plan *p, double *w, const YRows *rows, cudaStream_t st) {
+    const int complex_cols = (p->bcx == PP_BC_PERIODIC && p->bcy == PP_BC_PERIODIC) ? 1 : 0;
+#define CALL_Y(NN) launch_y_inv<NN>(w, p->nx / 2, p->nz, p->bcy, complex_cols, p->tw_y, p->ptw_y, rows, st)
+    PP_DISPATCH_N(p->ny, CALL_Y)
+#undef CALL_Y
+}
+
+}  // namespace pp

@@ -1,0 +1,109 @@
+// z-solve launcher (a7-a8): picks the partitioned, two-level or two-sweep kernels.
+#include <cmath>
+
+#include "pp_plan.h"
+#include "pp_zsolve.cuh"
+#include "pp_zpart.cuh"
+
+namespace pp {
+
+// The partitioned z kernels tabulate the leading minors q_0 .. q_R of a segment block, |q_R| <= bmax^R:
+// for grids so anisotropic (dz >> dx) that this could leave the fp64 range they are not used.
+bool zpart_range_ok(const pp_plan *p, int R) { return (double)R * std::log2(p->bmax) < 1000.0; }
+static ZPartShape plan_zpart_shape(const pp_plan *p) {
+    const ZPartShape z = zpart_shape(p->nz);
+    return (z.R && zpart_range_ok(p, z.R)) ? z : ZPartShape{0, 0, 0};
+}
+
+bool zpart_single_level(const pp_plan *p) { return plan_zpart_shape(p).R != 0; }
+
+int run_z(const pp_plan *p, double *w, cudaStream_t st) {
+    ZParams zp;
+    zp.nx = p->nx; zp.ny = p->ny; zp.nz = p->nz;
+    zp.bcz = p->bcz;
+    zp.singular = p->singular ? (p->null_space == PP_NULL_PIN_PLANE0 ? 2 : 1) : 0;
+    zp.scale = p->scale;
+    zp.sx = p->sx; zp.sy = p->sy;
+    zp.zero_scratch = p->zero_scratch;
+    const size_t plane = (size_t)p->nx * p->ny;
+#ifndef PP_Z_DSMEM
+#define PP_Z_DSMEM 0
+#endif
+#ifndef PP_Z_CB
+#define PP_Z_CB 16
+#endif
+    const bool want_part = p->z_algorithm != PP_Z_SWEEP;
+    const ZPartShape zs = want_part ? plan_zpart_shape(p) : ZPartShape{0, 0, 0};
+    if (zs.R) {
+        // partitioned, register-resident solve: one HBM read + one write per unknown (pp_zpart.cuh)
+        const bool cyc = p->bcz == PP_BC_PERIODIC;
+        const size_t ds = zpart_smem_bytes(zs, cyc);
+        const unsigned grid = (unsigned)((plane + zs.L - 1) / zs.L);
+        const ZHier none = {1, nullptr, nullptr};
+        auto launch = [&](auto kernel) -> int {
+            if (int rc = set_smem(kernel, ds)) return rc;
+            kernel<<<grid, zs.L * zs.S, ds, st>>>(w, zp, zs.S, zs.L, none);
+            return PP_SUCCESS;
+        };
+        int rc;
+        if (zs.R == 32) rc = cyc ? launch(zsolve_part_kernel<32, 0, true>) : launch(zsolve_part_kernel<32, 0, false>);
+        else            rc = cyc ? launch(zsolve_part_kernel<64, 0, true>) : launch(zsolve_part_kernel<64, 0, false>);
+        if (rc) return rc;
+    } else if (want_part && p->hier_scratch) {
+        // long lines: two-level partition, 8 + 16 bytes per unknown (pp_zpart.cuh, ZHier)
+        const ZPartShape hs = {32, ZP_HIER_ROWS / 32, 32};
+        const size_t ds = zpart_smem_bytes(hs);
+        const int nK = p->nz / ZP_HIER_ROWS;
+        const size_t slab = (size_t)nK * plane;
+        const ZHier h = {nK, p->hier_scratch, p->hier_scratch + slab};
+        const dim3 grid((unsigned)((plane + hs.L - 1) / hs.L), (unsigned)nK);
+        if (int rc = set_smem(zsolve_part_kernel<32, 1>, ds)) return rc;
+        if (int rc = set_smem(zsolve_part_kernel<32, 2>, ds)) return rc;
+        if (p->singular) {
+            // the singular (0,0) line touches column 0 only, which the passes below never store and whose
+            // values they discard: it runs beside them on the plan's side stream (fork / join by events)
+            if (cudaEventRecord(p->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(p->side, p->ev_fork, 0) != cudaSuccess) {
+                cudaGetLastError();
+                return PP_ERR_CUDA;
+            }
+            zero_mode_long_kernel<<<1, 1024, 0, p->side>>>(w, plane, p->nz, p->scale, p->null_space == PP_NULL_PIN_PLANE0);
+            if (cudaEventRecord(p->ev_join, p->side) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+        }
+        zsolve_part_kernel<32, 1><<<grid, hs.L * hs.S, ds, st>>>(w, zp, hs.S, hs.L, h);
+        zsolve_hier_interface_kernel<<<(unsigned)((plane + 63) / 64), 64, 0, st>>>(zp, h, ZP_HIER_ROWS, p->hier_scratch + 2 * slab,
+                                                                             p->hier_scratch + 3 * slab);
+        zsolve_part_kernel<32, 2><<<grid, hs.L * hs.S, ds, st>>>(w, zp, hs.S, hs.L, h);
+        if (p->singular && cudaStreamWaitEvent(st, p->ev_join, 0) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    } else if (p->bcz != PP_BC_PERIODIC) {
+        // checkpoint table in shared memory: ceil(nz / CB) x TH doubles per CTA
+#define PP_ZT_LAUNCH(C, T)                                                                           \
+        do {                                                                                         \
+            const size_t ds = (size_t)(((p->nz + 1) / 2 + C - 1) / C) * T * sizeof(double) + PP_Z_DSMEM; \
+            if (int rc = set_smem(zsolve_thomas_kernel<C, T>, ds)) return rc;                        \
+            zsolve_thomas_kernel<C, T><<<(unsigned)((plane + T - 1) / T), T, ds, st>>>(w, zp);       \
+        } while (0)
+#ifdef PP_Z_TH
+        PP_ZT_LAUNCH(PP_Z_CB, PP_Z_TH);
+#else
+        PP_ZT_LAUNCH(PP_Z_CB, 128);
+#endif
+#undef PP_ZT_LAUNCH
+    } else {
+        constexpr int TH = PP_Z_THREADS;
+        const unsigned grid = (unsigned)((plane + TH - 1) / TH);
+        const int cb = (p->nz <= 16 * Z_MAX_CK) ? 16 : ((p->nz <= 32 * Z_MAX_CK) ? 32 : 64);
+        const size_t ds = PP_Z_DSMEM;      // dummy dynamic shared memory: caps resident CTAs per SM
+#define PP_Z_LAUNCH(K, C)                                                                        \
+        do {                                                                                     \
+            if (int rc = set_smem(K<C>, ds)) return rc;                                          \
+            K<C><<<grid, TH, ds, st>>>(w, zp);                                                   \
+        } while (0)
+        if (cb == 16)      PP_Z_LAUNCH(zsolve_cyclic_kernel, 16);
+        else if (cb == 32) PP_Z_LAUNCH(zsolve_cyclic_kernel, 32);
+        else               PP_Z_LAUNCH(zsolve_cyclic_kernel, 64);
+#undef PP_Z_LAUNCH
+    }
+    return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
+}
+
+}  // namespace pp

@@ -46,13 +46,19 @@ __device__ __forceinline__ double sgn_of(int i) { return (i & 1) ? -1.0 : 1.0; }
 #define PP_X_MINB 4
 #endif
 
+#ifndef PP_X_E16_MIN
+#define PP_X_E16_MIN 4096     // x pass: 16 elements per thread from this length on (4096: never)
+#endif
+
 template <int N>
 struct XCfg {
-    static constexpr int P = FftCfg<N>::P;
+    static constexpr int E = fft_E(N, PP_X_E16_MIN);
+    using F = FftCfg<N, E>;
+    static constexpr int P = F::P;
     static constexpr int T = (256 / P) > 0 ? (256 / P) : 1;   // transforms (row pairs) per CTA; <= 4 when P >= 64
     static constexpr int THREADS = T * P;
-    static constexpr int MINB = (FftCfg<N>::E <= 12) ? PP_X_MINB : 2;   // 20 elements per thread need more than 64 registers
-    static constexpr size_t SMEM = size_t(T) * FftCfg<N>::SMEM_ELEMS * sizeof(double2);
+    static constexpr int MINB = (E <= 12) ? PP_X_MINB : 2;    // 16 or 20 elements per thread need more than 64 registers
+    static constexpr size_t SMEM = size_t(T) * F::SMEM_ELEMS * sizeof(double2);
 };
 
 // ------------------------------------------------------------------------------------------
@@ -64,7 +70,7 @@ template <int N, int T>
 __device__ __forceinline__ void xfwd_tile(const double *in, double *out, long long pair0, long long npairs, int bc,
                                           const double2 *__restrict__ tw, const double2 *__restrict__ ptw,
                                           double2 *smem) {
-    using C = FftCfg<N>;
+    using C = typename XCfg<N>::F;
     constexpr int E = C::E, P = C::P, H = N / 2;
     const int f = threadIdx.x / P, t = threadIdx.x % P;
     const long long pair = pair0 + f;
@@ -171,7 +177,7 @@ template <int N, int T, bool LDCG>
 __device__ __forceinline__ void xinv_tile(const double *in, double *out, long long pair0, long long npairs, int bc,
                                           const double2 *__restrict__ tw, const double2 *__restrict__ ptw,
                                           double2 *smem) {
-    using C = FftCfg<N>;
+    using C = typename XCfg<N>::F;
     constexpr int E = C::E, P = C::P, H = N / 2;
     const int f = threadIdx.x / P, t = threadIdx.x % P;
     const long long pair = pair0 + f;

@@ -32,22 +32,20 @@ struct LayoutCol {
     __device__ __forceinline__ int operator()(int i) const { return pad8(i) * T + c; }
 };
 
-// Tiles of 4 columns (N > 512): a quarter-warp -- the unit a 16-byte shared-memory access is served
-// in -- is 4 columns x 2 consecutive rows (t even, t + 1), so the two rows must land in different halves
-// of a 128-byte bank row.  The padded layout does that for the row patterns of radix-8 stages only; the
-// leading radix-2 / radix-4 stage of the 1024- and 2048-point transforms stores rows that differ by
-// R0 = 2^S and conflicts two-way.  Here the low bit of the row is XORed with bit S instead: rows i, i+1
-// (i even: every load, every later store) and rows i, i + R0 (the first stage's stores) then always differ
-// in that bit.  No padding needed.
-template <int S>
-struct LayoutColXor4 {
+// Tiles of fewer than 8 columns (N > 512).  A quarter-warp -- the unit a 16-byte shared-memory access is
+// served in -- is T columns x 8/T consecutive rows (t aligned to 8/T), so those 8/T rows must land in
+// different T*16-byte slices of a 128-byte bank row.  The padded layout does that for the row patterns of
+// radix-8 stages on 8 columns only.  Here the low log2(8/T) bits of the row are XORed with the bits just
+// above the first radix R0 = 2^S instead:
+//   loads (rows t + m P) and the stores of every later stage (rows .. + k, k = t mod NS): the 8/T rows are
+//     consecutive and share the XORed bits -- still distinct;
+//   stores of the first stage (rows t R0 + r): the rows differ in exactly the bits S.. that are XORed in.
+// No padding needed.
+template <int T, int S>
+struct LayoutColXor {
+    static constexpr int MASK = 8 / T - 1;
     int c;
-    __device__ __forceinline__ int operator()(int i) const { return ((i ^ ((i >> S) & 1)) << 2) + c; }
-};
-template <int N, int T>
-struct YLayout {
-    static constexpr bool XOR4 = (T == 4) && ((N & (N - 1)) == 0) && (FftCfg<N>::R0 == 2 || FftCfg<N>::R0 == 4);
-    using type = typename std::conditional<XOR4, LayoutColXor4<FftCfg<N>::R0 == 2 ? 1 : 2>, LayoutCol<T>>::type;
+    __device__ __forceinline__ int operator()(int i) const { return (i ^ ((i >> S) & MASK)) * T + c; }
 };
 
 struct SyncCta {
@@ -57,17 +55,31 @@ struct SyncCta {
 #ifndef PP_Y_T
 #define PP_Y_T 8          // double2 columns per CTA for N <= 512 (128-byte row segments)
 #endif
+#ifndef PP_Y_T_1024
+#define PP_Y_T_1024 4     // ... for N in (512, 1024]
+#endif
+#ifndef PP_Y_T_2048
+#define PP_Y_T_2048 4     // ... for N > 1024
+#endif
 #ifndef PP_Y_MINB
 #define PP_Y_MINB 2       // __launch_bounds__ min CTAs per SM (caps registers) for CTAs of <= 512 threads
+#endif
+#ifndef PP_Y_E16_MIN
+#define PP_Y_E16_MIN 1024 // y pass: 16 elements per thread (radix-16 stages) from this length on
 #endif
 
 template <int N>
 struct YCfg {
-    static constexpr int P = FftCfg<N>::P;
-    static constexpr int T = (N <= 512) ? PP_Y_T : 4;   // double2 columns per CTA
+    static constexpr int E = fft_E(N, PP_Y_E16_MIN);
+    using F = FftCfg<N, E>;
+    static constexpr int P = F::P;
+    static constexpr int T = (N <= 512) ? PP_Y_T : ((N <= 1024) ? PP_Y_T_1024 : PP_Y_T_2048);   // double2 columns per CTA
     static constexpr int THREADS = T * P;
-    static constexpr int MINB = (THREADS <= 512) ? PP_Y_MINB : 1;
-    static constexpr size_t SMEM = size_t(T) * FftCfg<N>::SMEM_ELEMS * sizeof(double2);
+    // registers: 8 elements per thread fit 64 (two CTAs of 512 threads per SM); 16 or 20 need up to 128
+    static constexpr int MINB = (E <= 12) ? ((THREADS <= 512) ? PP_Y_MINB : 1) : ((THREADS <= 256) ? 2 : 1);
+    static constexpr bool XOR = (T < 8) && ((N & (N - 1)) == 0) && (N > 512);
+    using Layout = typename std::conditional<XOR, LayoutColXor<T, ilog2(F::R0)>, LayoutCol<T>>::type;
+    static constexpr size_t SMEM = size_t(T) * (XOR ? N : F::SMEM_ELEMS) * sizeof(double2);
 };
 
 __device__ __forceinline__ double2 dscale(double a, double2 v) { return make_double2(a * v.x, a * v.y); }
@@ -75,22 +87,43 @@ __device__ __forceinline__ double2 dscale(double a, double2 v) { return make_dou
 template <bool LDCG>
 __device__ __forceinline__ double2 yld(const double2 *p) { return LDCG ? __ldcg(p) : *p; }
 
+// Slab decomposition over several GPUs (pp_slab_*): the y pass is where the data is
+// re-oriented between z-slabs (x and y transforms local) and (kx, ky)-pencils (z solve local),
+// so the exchange is fused into it -- the forward pass STORES row j of plane z straight into the pencil
+// buffer of the rank that owns ky = j (a peer pointer over NVLink, or a chunk of a local all-to-all send
+// buffer), the inverse pass LOADS it from there.  Block b = j / rpb of `rpb` consecutive rows lives at
+// base[b], laid out [plane z][row j - b rpb][nxh]: with one block (rpb = ny) this is the plain array.
+constexpr int PP_MAX_WORLD = 16;
+struct YRows {
+    double2 *base[PP_MAX_WORLD];
+    int rpb;
+    __device__ __forceinline__ double2 *row(int z, int j, int ld) const {
+        const int b = j / rpb;
+        return base[b] + ((size_t)z * rpb + (j - b * rpb)) * (size_t)ld;
+    }
+};
+
 // One CTA-wide tile of the forward y pass: column tile bx (T double2 columns) of plane z, all N rows
-// (blockDim.x == T * FftCfg<N>::P).  `smem` holds T * FftCfg<N>::SMEM_ELEMS double2.  LDCG: read with
+// (blockDim.x == YCfg<N>::THREADS).  `smem` holds YCfg<N>::SMEM bytes.  LDCG: read with
 // ld.global.cg -- for the fused x+y kernel, whose input was just written by other SMs.
-template <int N, bool LDCG>
+template <int N, bool LDCG, bool SLAB = false>
 __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int complex_cols,
                                           const double2 *__restrict__ tw, const double2 *__restrict__ ptw,
-                                          int bx, int z, double2 *smem) {
-    using C = FftCfg<N>;
+                                          int bx, int z, double2 *smem, const YRows *rows = nullptr) {
+    using C = typename YCfg<N>::F;
     constexpr int E = C::E, P = C::P, T = YCfg<N>::T, H = N / 2;
     const int c = threadIdx.x % T, t = threadIdx.x / T;
     const int cp = bx * T + c;
     const bool active = cp < nxh;
     double2 *base = w + (size_t)z * N * nxh + (active ? cp : 0);
     const int ld = nxh;                                    // row offsets inside a plane fit 32 bits
-    const typename YLayout<N, T>::type lay{c};
+    const typename YCfg<N>::Layout lay{c};
     const SyncCta sync;
+    // where row j of the result goes: in place, or (slab decomposition) into the owner rank's pencil block
+    const auto out = [&](int j) -> double2 * {
+        if constexpr (SLAB) return rows->row(z, j, ld) + (active ? cp : 0);
+        else return base + j * ld;
+    };
 
     double2 v[E];
 #pragma unroll
@@ -112,7 +145,7 @@ __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int compl
     if (complex_cols && bx > 0) {                  // block-uniform: all columns complex
         if (active) {
 #pragma unroll
-            for (int q = 0; q < E; ++q) base[(t + q * P) * ld] = v[q];
+            for (int q = 0; q < E; ++q) *out((t + q * P)) = v[q];
         }
         return;
     }
@@ -122,7 +155,7 @@ __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int compl
     if (!active) return;
     if (complex_cols && cp > 0) {
 #pragma unroll
-        for (int q = 0; q < E; ++q) base[(t + q * P) * ld] = v[q];
+        for (int q = 0; q < E; ++q) *out((t + q * P)) = v[q];
         return;
     }
 #pragma unroll
@@ -133,34 +166,34 @@ __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int compl
         if (m == 0) {
             const double2 zh = v[E / 2];
             if (bc == BC_P) {
-                base[0] = zm;
-                base[H * ld] = zh;
+                *out(0) = zm;
+                *out(H) = zh;
             } else {
                 const double c4 = ptw[H].x;
                 if (bc == BC_N) {
-                    base[0] = zm;
-                    base[H * ld] = dscale(c4, zh);
+                    *out(0) = zm;
+                    *out(H) = dscale(c4, zh);
                 } else {
-                    base[(N - 1) * ld] = dscale(-1.0, zm);
-                    base[(N - 1 - H) * ld] = dscale(-sgn_of(H) * c4, zh);
+                    *out((N - 1)) = dscale(-1.0, zm);
+                    *out((N - 1 - H)) = dscale(-sgn_of(H) * c4, zh);
                 }
             }
         } else {
             const double2 A = make_double2(0.5 * (zm.x + zc.x), 0.5 * (zm.y - zc.y));
             const double2 B = make_double2(0.5 * (zm.y + zc.y), -0.5 * (zm.x - zc.x));
             if (bc == BC_P) {
-                base[m * ld] = make_double2(A.x, B.x);
-                base[(N - m) * ld] = make_double2(A.y, B.y);
+                *out(m) = make_double2(A.x, B.x);
+                *out((N - m)) = make_double2(A.y, B.y);
             } else {
                 const double2 wm = __ldg(&ptw[m]);
                 const double2 ca = cmul(wm, A), cb = cmul(wm, B);
                 if (bc == BC_N) {
-                    base[m * ld] = make_double2(ca.x, cb.x);
-                    base[(N - m) * ld] = make_double2(-ca.y, -cb.y);
+                    *out(m) = make_double2(ca.x, cb.x);
+                    *out((N - m)) = make_double2(-ca.y, -cb.y);
                 } else {
                     const double s1 = -sgn_of(m);
-                    base[(N - 1 - m) * ld] = make_double2(s1 * ca.x, s1 * cb.x);
-                    base[(m - 1) * ld] = make_double2(-s1 * ca.y, -s1 * cb.y);
+                    *out((N - 1 - m)) = make_double2(s1 * ca.x, s1 * cb.x);
+                    *out((m - 1)) = make_double2(-s1 * ca.y, -s1 * cb.y);
                 }
             }
         }
@@ -178,26 +211,40 @@ ypass_fwd_kernel(double2 *w, int nxh, int bc, int complex_cols,
     yfwd_tile<N, false>(w, nxh, bc, complex_cols, tw, ptw, blockIdx.x, gridDim.y - 1 - blockIdx.y, smem);
 }
 
-// One CTA-wide tile of the inverse y pass (see yfwd_tile).
+// slab decomposition: reads the local z-slab w, stores every row into the pencil block of the rank that owns it
 template <int N>
+__global__ void __launch_bounds__(YCfg<N>::THREADS, YCfg<N>::MINB)
+ypass_fwd_slab_kernel(double2 *w, int nxh, int bc, int complex_cols,
+                      const double2 *__restrict__ tw, const double2 *__restrict__ ptw, const __grid_constant__ YRows rows) {
+    extern __shared__ double2 smem[];
+    yfwd_tile<N, false, true>(w, nxh, bc, complex_cols, tw, ptw, blockIdx.x, gridDim.y - 1 - blockIdx.y, smem, &rows);
+}
+
+// One CTA-wide tile of the inverse y pass (see yfwd_tile).
+template <int N, bool SLAB = false>
 __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int complex_cols,
                                           const double2 *__restrict__ tw, const double2 *__restrict__ ptw,
-                                          int bx, int z, double2 *smem) {
-    using C = FftCfg<N>;
+                                          int bx, int z, double2 *smem, const YRows *rows = nullptr) {
+    using C = typename YCfg<N>::F;
     constexpr int E = C::E, P = C::P, T = YCfg<N>::T, H = N / 2;
     const int c = threadIdx.x % T, t = threadIdx.x / T;
     const int cp = bx * T + c;
     const bool active = cp < nxh;
     double2 *base = w + (size_t)z * N * nxh + (active ? cp : 0);
     const int ld = nxh;                                    // row offsets inside a plane fit 32 bits
-    const typename YLayout<N, T>::type lay{c};
+    const typename YCfg<N>::Layout lay{c};
     const SyncCta sync;
     const bool cplx = complex_cols && cp > 0;
+    // where row j of the input comes from: in place, or (slab decomposition) the owner rank's pencil block
+    const auto in = [&](int j) -> const double2 * {
+        if constexpr (SLAB) return rows->row(z, j, ld) + (active ? cp : 0);
+        else return base + j * ld;
+    };
 
     double2 v[E];
     if (complex_cols && bx > 0) {                          // block-uniform: every column of the tile is complex
 #pragma unroll
-        for (int q = 0; q < E; ++q) v[q] = base[(t + q * P) * ld];
+        for (int q = 0; q < E; ++q) v[q] = *in((t + q * P));
     } else {
         // Real pairs: row m and row N-m are needed together, for V_m and for V_{N-m}.  The owner of
         // m in [0, N/2) loads the two rows once, keeps V_m and hands V_{N-m} to its owner through shared
@@ -210,16 +257,16 @@ __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int compl
         for (int q = 0; q < E / 2; ++q) {
             const int m = t + q * P;                       // 0 <= m < N/2
             if (cplx) {
-                v[q] = base[m * ld];
-                v[q + E / 2] = base[(m + H) * ld];
+                v[q] = *in(m);
+                v[q + E / 2] = *in((m + H));
             } else if (bc == BC_P || bc == BC_N) {
-                v[q] = base[m * ld];
-                v[q + E / 2] = (m > 0) ? base[(N - m) * ld] : make_double2(0.0, 0.0);
-                if (m == 0) yh = base[H * ld];
+                v[q] = *in(m);
+                v[q + E / 2] = (m > 0) ? *in((N - m)) : make_double2(0.0, 0.0);
+                if (m == 0) yh = *in(H);
             } else {
-                v[q] = base[(N - 1 - m) * ld];
-                v[q + E / 2] = (m > 0) ? base[(m - 1) * ld] : make_double2(0.0, 0.0);
-                if (m == 0) yh = base[(N - 1 - H) * ld];
+                v[q] = *in((N - 1 - m));
+                v[q + E / 2] = (m > 0) ? *in((m - 1)) : make_double2(0.0, 0.0);
+                if (m == 0) yh = *in((N - 1 - H));
             }
         }
         if (!cplx) {
@@ -281,6 +328,15 @@ ypass_inv_kernel(double2 *w, int nxh, int bc, int complex_cols,
                  const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
     extern __shared__ double2 smem[];
     yinv_tile<N>(w, nxh, bc, complex_cols, tw, ptw, blockIdx.x, blockIdx.y, smem);
+}
+
+// slab decomposition: loads every row from the pencil block of the rank that owns it, stores the local z-slab w
+template <int N>
+__global__ void __launch_bounds__(YCfg<N>::THREADS, YCfg<N>::MINB)
+ypass_inv_slab_kernel(double2 *w, int nxh, int bc, int complex_cols,
+                      const double2 *__restrict__ tw, const double2 *__restrict__ ptw, const __grid_constant__ YRows rows) {
+    extern __shared__ double2 smem[];
+    yinv_tile<N, true>(w, nxh, bc, complex_cols, tw, ptw, blockIdx.x, blockIdx.y, smem, &rows);
 }
 
 }  // namespace pp

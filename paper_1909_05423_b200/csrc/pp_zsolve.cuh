@@ -24,6 +24,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include "pp_zshape.h"
 
 namespace pp {
 
@@ -38,7 +39,6 @@ struct ZParams {
     double *zero_scratch;    // [nz]  scratch line for the zero-mode solve
 };
 
-constexpr int Z_MAX_CK = 64;   // checkpoints per line
 
 // L2 eviction-priority hints (createpolicy + .L2::cache_hint).  The forward sweep's x' values are
 // re-read by the backward sweep: they are stored "evict_last" so they survive in the 126 MB L2,

@@ -133,13 +133,16 @@ def config2(combo: str, variant: str = "mms", n: int = 128) -> Workload:
     return Workload(f"cfg2-{n}^3-{combo}-normal", shape, h, bc, f)
 
 
-def config3(scale: int = 1) -> Workload:
+def config3(scale: int = 1, combo: str = "PPN") -> Workload:
     """512 x 512 x 256, periodic x/y, Neumann z, unit cube; N(0,1) projected to zero mean.
-    ``scale`` > 1 divides every extent (for quick CPU-sized siblings of the headline grid)."""
+    ``scale`` > 1 divides every extent (for quick CPU-sized siblings of the headline grid); ``combo`` other
+    than 'PPN' keeps grid, spacings and seed and changes the boundary conditions only (the same field,
+    projected to zero mean when the combination is singular) -- for per-BC timings at the headline size."""
     nx, ny, nz = 512 // scale, 512 // scale, 256 // scale
-    shape, h, bc = (nz, ny, nx), (1.0 / nx, 1.0 / ny, 1.0 / nz), (P, P, N)
-    f = random_normal(shape, seed_for(3, 0), zero_mean=True)
-    return Workload(f"cfg3-{nx}x{ny}x{nz}-PPN-normal", shape, h, bc, f)
+    bc = parse_bc(combo)
+    shape, h = (nz, ny, nx), (1.0 / nx, 1.0 / ny, 1.0 / nz)
+    f = random_normal(shape, seed_for(3, 0), zero_mean=all(b in (P, N) for b in bc))
+    return Workload(f"cfg3-{nx}x{ny}x{nz}-{combo.upper()}-normal", shape, h, bc, f)
 
 
 def paper_pencil(combo: str = "PPN", nxy: int = 64, nz: int = 16384) -> Workload:

@@ -25,11 +25,11 @@ def solve(f, h, bc, fusion, in_place=False):
     return u
 
 
-@pytest.mark.parametrize("n", [128, 256, 512, 1024])
+@pytest.mark.parametrize("n", [128, 256, 512])
 @pytest.mark.parametrize("combo", ["PPN", "NND", "DDD", "PNP", "DPN", "NNN"])
 def test_fused_is_bit_identical_and_matches_oracle(n, combo):
     bc = wl.parse_bc(combo)
-    nz = {128: 37, 256: 12, 512: 7, 1024: 3}[n]          # several lags' worth of planes at the small sizes
+    nz = {128: 37, 256: 12, 512: 7}[n]          # several lags' worth of planes at the small sizes
     shape = (nz, n, n)
     h = (1.0 / n, 0.9 / n, 1.0 / 16)
     f = wl.random_normal(shape, 500 + n, zero_mean=all(b in (0, 1) for b in bc))
