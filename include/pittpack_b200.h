@@ -67,9 +67,9 @@ enum { PP_K_XFWD = 0, PP_K_YFWD = 1, PP_K_ZSOLVE = 2, PP_K_YINV = 3, PP_K_XINV =
  * "assignBoundary(bc)" (Listing 3).
  *   out      : host pointer receiving the handle (set to NULL on failure).
  *   nx, ny   : 2^k in [4, 2048], 3 * 2^k in [48, 1536] or 5 * 2^k in [80, 1280] (the hand-written FFT
- *              core; the 48-multiples are the paper's weak-scaling grids);  nz in [2, 4096], or -- with
- *              Neumann / Dirichlet z -- any multiple of 256 up to 16384 (the paper's 64 x 64 x 16384
- *              pencils; solved by the two-level partition, see pp_plan_set_z_algorithm).
+ *              core; the 48-multiples are the paper's weak-scaling grids);  nz in [2, 16384], any
+ *              boundary condition (16384: the paper's 64 x 64 x 16384 pencils).  Which z kernel
+ *              serves which nz: pp_plan_set_z_algorithm.
  * Synchronous.  Builds the twiddle, post-twiddle and modified-wavenumber tables on the host
  * in extended precision and uploads them to the CURRENT device; the plan is bound to it.
  */
@@ -127,17 +127,18 @@ int pp_plan_last_kernel_ms(pp_plan *plan, float *ms_out);
  * tridiagonal algorithm open and offers several).  Both compute the same
  * Thomas elimination of Algorithm 2 up to rounding order.
  *   PP_Z_AUTO      : partitioned where it applies, two-sweep otherwise (the default).
- *   PP_Z_SWEEP     : two-sweep Thomas, one thread per system, any nz <= 4096; periodic z by
- *                    Sherman-Morrison.
+ *   PP_Z_SWEEP     : two-sweep Thomas, one thread per system, any nz; periodic z by
+ *                    Sherman-Morrison.  (Beyond 4096 rows it runs 32 threads per CTA: a
+ *                    fallback for line lengths the partition does not take, not a fast path.)
  *   PP_Z_PARTITION : each system cut into segments of 32 or 64 rows held in registers and
  *                    coupled through their interface unknowns (the reduction idea of CR-P,
  *                    PAPER.md:250-258, across the threads of one CTA); with periodic z the
  *                    interface chain closes on itself (a 2x2 closure instead of Sherman-Morrison's
- *                    second solve).  Needs nz = 32 m or 64 m (m <= 8), 1024 or 2048 -- or, for
- *                    Neumann / Dirichlet z, nz = 256 m (2 <= m <= 64), where the same partition is
- *                    applied on two levels (super-segments of 256 rows, three kernels); otherwise
- *                    PP_ERR_UNSUPPORTED_SIZE and the plan is left unchanged.  PP_Z_SWEEP is
- *                    refused for nz > 4096.  The partitioned kernels tabulate segment
+ *                    second solve).  Needs nz = 32 m or 64 m (m <= 8), 1024 or 2048 -- or
+ *                    nz = 256 m (2 <= m <= 64), where the same partition is applied on two levels
+ *                    (super-segments of 256 rows, three kernels; with periodic z the chain of
+ *                    super-segments closes on itself the same way); otherwise
+ *                    PP_ERR_UNSUPPORTED_SIZE and the plan is left unchanged.  The partitioned kernels tabulate segment
  *                    determinants of magnitude up to (3 + max|s|)^R (R = 32 or 64 rows per
  *                    segment, s the spectral shift dz^2 (lam_x/dx^2 + lam_y/dy^2)); grids so
  *                    anisotropic that this could leave the fp64 range (dz/dx beyond ~90 with

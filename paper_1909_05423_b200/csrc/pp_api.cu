@@ -6,9 +6,10 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
 #include <mutex>
 #include <new>
-#include <set>
+#include <utility>
 #include <vector>
 
 #include "pp_plan.h"
@@ -19,28 +20,21 @@
 using namespace pp;
 
 namespace pp {
-struct SmemKey {
-    int device; const void *fn; size_t smem;
-    bool operator<(const SmemKey &o) const {
-        if (device != o.device) return device < o.device;
-        if (fn != o.fn) return fn < o.fn;
-        return smem < o.smem;
-    }
-};
+// largest dynamic shared-memory size each (device, kernel) has been opted in to: the attribute is only ever raised
 static std::mutex g_smem_mutex;
-static std::set<SmemKey> g_smem_done;
+static std::map<std::pair<int, const void *>, size_t> g_smem_max;
 
 int set_smem_once(const void *kernel, size_t smem) {
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
-    const SmemKey key{dev, kernel, smem};
     std::lock_guard<std::mutex> lock(g_smem_mutex);
-    if (g_smem_done.count(key)) return PP_SUCCESS;
+    size_t &have = g_smem_max[std::make_pair(dev, kernel)];
+    if (smem <= have) return PP_SUCCESS;
     if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
         cudaGetLastError();
         return PP_ERR_CUDA;
     }
-    g_smem_done.insert(key);
+    have = smem;
     return PP_SUCCESS;
 }
 }  // namespace pp
@@ -51,6 +45,8 @@ int set_smem_once(const void *kernel, size_t smem) {
 namespace {
 
 const long double PI_L = 3.14159265358979323846264338327950288L;
+
+constexpr int PP_MAX_NZ = 16384;        // longest z line (the paper's pencils)
 
 // powers of two in [4, 2048], 3 * 2^k in [48, 1536], 5 * 2^k in [80, 1280]
 bool length_supported(int n) { return n >= 4 && n <= 2048 && fft_length_ok(n); }
@@ -150,7 +146,7 @@ const char *pp_strerror(int status) {
     switch (status) {
         case PP_SUCCESS: return "success";
         case PP_ERR_INVALID_ARG: return "invalid argument";
-        case PP_ERR_UNSUPPORTED_SIZE: return "unsupported grid size (nx, ny: 2^k in [4, 2048], 3*2^k in [48, 1536] or 5*2^k in [80, 1280]; nz in [2, 4096], or 256 m <= 16384 with non-periodic z)";
+        case PP_ERR_UNSUPPORTED_SIZE: return "unsupported grid size (nx, ny: 2^k in [4, 2048], 3*2^k in [48, 1536] or 5*2^k in [80, 1280]; nz in [2, 16384])";
         case PP_ERR_ALLOC: return "allocation failed";
         case PP_ERR_CUDA: return "CUDA runtime or launch error (is a CUDA device present?)";
         case PP_ERR_NULL: return "null pointer argument";
@@ -167,10 +163,10 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
         return PP_ERR_INVALID_ARG;
     for (int bc : {bc_x, bc_y, bc_z})
         if (bc != PP_BC_PERIODIC && bc != PP_BC_NEUMANN && bc != PP_BC_DIRICHLET) return PP_ERR_INVALID_ARG;
-    // nz: the two-sweep kernels take any nz up to 4096; longer lines need the two-level partition
-    // (Neumann / Dirichlet z, nz a multiple of 256 up to 16384)
-    const bool long_ok = bc_z != PP_BC_PERIODIC && zpart_hier_ok(nz);
-    if (!length_supported(nx) || !length_supported(ny) || nz < 2 || (nz > 64 * Z_MAX_CK && !long_ok)) return PP_ERR_UNSUPPORTED_SIZE;
+    // nz: any value in [2, 16384].  Multiples of 256 beyond what one CTA holds go to the two-level partition,
+    // everything the partitioned kernels do not take to the two-sweep kernels.
+    const bool long_ok = zpart_hier_ok(nz);
+    if (!length_supported(nx) || !length_supported(ny) || nz < 2 || nz > PP_MAX_NZ) return PP_ERR_UNSUPPORTED_SIZE;
 
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
@@ -208,15 +204,15 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
     { double m = 0.0; for (double v : s) m = v < m ? v : m; smin += m; }
     if (!rc) rc = upload(&p->sy, s, p->bytes);
     p->bmax = 3.0 - smin;
-    // lines beyond the two-sweep kernel's range need the two-level partition (segments of 32 rows)
-    // (its interface kernel carries the minors over 33 rows before the first renormalisation)
-    if (!rc && nz > 64 * Z_MAX_CK && !zpart_range_ok(p, 33)) rc = PP_ERR_UNSUPPORTED_SIZE;
     if (!rc) {
         std::vector<double> z((size_t)nz, 0.0);
         rc = upload(&p->zero_scratch, z, p->bytes);
     }
+    // two-level partition (segments of 32 rows; its interface kernels carry the minors over up to 33 rows between
+    // renormalisations, hence the range check): interface values [2][nK][plane] + scratch [2][nK][plane], or
+    // [6][nK][plane] when the chain of super-segments is cyclic (periodic z)
     if (!rc && long_ok && zpart_shape(nz).R == 0 && zpart_range_ok(p, 33)) {
-        const size_t nb = sizeof(double) * 4 * (size_t)(nz / ZP_HIER_ROWS) * (size_t)nx * (size_t)ny;
+        const size_t nb = sizeof(double) * (bc_z == PP_BC_PERIODIC ? 8 : 4) * (size_t)(nz / ZP_HIER_ROWS) * (size_t)nx * (size_t)ny;
         if (cudaMalloc((void **)&p->hier_scratch, nb) != cudaSuccess) { p->hier_scratch = nullptr; cudaGetLastError(); rc = PP_ERR_ALLOC; }
         else p->bytes += nb;
     }
@@ -468,7 +464,6 @@ int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm) {
     if (algorithm != PP_Z_AUTO && algorithm != PP_Z_SWEEP && algorithm != PP_Z_PARTITION) return PP_ERR_INVALID_ARG;
     if (algorithm == PP_Z_PARTITION && !zpart_single_level(plan) && !plan->hier_scratch)
         return PP_ERR_UNSUPPORTED_SIZE;
-    if (algorithm == PP_Z_SWEEP && plan->nz > 64 * Z_MAX_CK) return PP_ERR_UNSUPPORTED_SIZE;
     plan->z_algorithm = algorithm;
     return PP_SUCCESS;
 }
@@ -512,8 +507,7 @@ int pp_plan_set_null_space(pp_plan *plan, int convention) {
 
 int pp_size_supported(int nx, int ny, int nz, int bc_z) {
     if (bc_z != PP_BC_PERIODIC && bc_z != PP_BC_NEUMANN && bc_z != PP_BC_DIRICHLET) return 0;
-    const bool long_ok = bc_z != PP_BC_PERIODIC && zpart_hier_ok(nz);
-    return (length_supported(nx) && length_supported(ny) && nz >= 2 && (nz <= 64 * Z_MAX_CK || long_ok)) ? 1 : 0;
+    return (length_supported(nx) && length_supported(ny) && nz >= 2 && nz <= PP_MAX_NZ) ? 1 : 0;
 }
 
 int pp_plan_launches_per_solve(const pp_plan *plan) {

@@ -39,7 +39,7 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
         const bool cyc = p->bcz == PP_BC_PERIODIC;
         const size_t ds = zpart_smem_bytes(zs, cyc);
         const unsigned grid = (unsigned)((plane + zs.L - 1) / zs.L);
-        const ZHier none = {1, nullptr, nullptr};
+        const ZHier none = {1, nullptr, nullptr, 0};
         auto launch = [&](auto kernel) -> int {
             if (int rc = set_smem(kernel, ds)) return rc;
             kernel<<<grid, zs.L * zs.S, ds, st>>>(w, zp, zs.S, zs.L, none);
@@ -55,7 +55,8 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
         const size_t ds = zpart_smem_bytes(hs);
         const int nK = p->nz / ZP_HIER_ROWS;
         const size_t slab = (size_t)nK * plane;
-        const ZHier h = {nK, p->hier_scratch, p->hier_scratch + slab};
+        const bool per = p->bcz == PP_BC_PERIODIC;
+        const ZHier h = {nK, p->hier_scratch, p->hier_scratch + slab, per ? 1 : 0};
         const dim3 grid((unsigned)((plane + hs.L - 1) / hs.L), (unsigned)nK);
         if (int rc = set_smem(zsolve_part_kernel<32, 1>, ds)) return rc;
         if (int rc = set_smem(zsolve_part_kernel<32, 2>, ds)) return rc;
@@ -66,22 +67,29 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
                 cudaGetLastError();
                 return PP_ERR_CUDA;
             }
-            zero_mode_long_kernel<<<1, 1024, 0, p->side>>>(w, plane, p->nz, p->scale, p->null_space == PP_NULL_PIN_PLANE0);
+            zero_mode_long_kernel<<<1, 1024, 0, p->side>>>(w, plane, p->nz, p->scale, p->null_space == PP_NULL_PIN_PLANE0, per ? 1 : 0);
             if (cudaEventRecord(p->ev_join, p->side) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
         }
         zsolve_part_kernel<32, 1><<<grid, hs.L * hs.S, ds, st>>>(w, zp, hs.S, hs.L, h);
-        zsolve_hier_interface_kernel<<<(unsigned)((plane + 63) / 64), 64, 0, st>>>(zp, h, ZP_HIER_ROWS, p->hier_scratch + 2 * slab,
-                                                                             p->hier_scratch + 3 * slab);
+        if (per)
+            zsolve_hier_interface_cyclic_kernel<<<(unsigned)((plane + 63) / 64), 64, 0, st>>>(zp, h, ZP_HIER_ROWS, p->hier_scratch + 2 * slab);
+        else
+            zsolve_hier_interface_kernel<<<(unsigned)((plane + 63) / 64), 64, 0, st>>>(zp, h, ZP_HIER_ROWS, p->hier_scratch + 2 * slab,
+                                                                                 p->hier_scratch + 3 * slab);
         zsolve_part_kernel<32, 2><<<grid, hs.L * hs.S, ds, st>>>(w, zp, hs.S, hs.L, h);
         if (p->singular && cudaStreamWaitEvent(st, p->ev_join, 0) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
     } else if (p->bcz != PP_BC_PERIODIC) {
-        // checkpoint table in shared memory: ceil(nz / CB) x TH doubles per CTA
+        // two-sweep Thomas; checkpoint table in shared memory: ceil(ceil(nz / 2) / CB) x TH doubles per CTA.
+        // Lines beyond 4096 rows that the two-level partition does not take (nz not a multiple of 256) run with
+        // 32 threads per CTA so that their 512 checkpoints per system still fit: slow, but every nz <= 16384 solves.
 #define PP_ZT_LAUNCH(C, T)                                                                           \
         do {                                                                                         \
             const size_t ds = (size_t)(((p->nz + 1) / 2 + C - 1) / C) * T * sizeof(double) + PP_Z_DSMEM; \
             if (int rc = set_smem(zsolve_thomas_kernel<C, T>, ds)) return rc;                        \
             zsolve_thomas_kernel<C, T><<<(unsigned)((plane + T - 1) / T), T, ds, st>>>(w, zp);       \
         } while (0)
+        if (p->nz > 64 * Z_MAX_CK) PP_ZT_LAUNCH(16, 32);
+        else
 #ifdef PP_Z_TH
         PP_ZT_LAUNCH(PP_Z_CB, PP_Z_TH);
 #else
@@ -89,18 +97,18 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
 #endif
 #undef PP_ZT_LAUNCH
     } else {
-        constexpr int TH = PP_Z_THREADS;
-        const unsigned grid = (unsigned)((plane + TH - 1) / TH);
-        const int cb = (p->nz <= 16 * Z_MAX_CK) ? 16 : ((p->nz <= 32 * Z_MAX_CK) ? 32 : 64);
-        const size_t ds = PP_Z_DSMEM;      // dummy dynamic shared memory: caps resident CTAs per SM
-#define PP_Z_LAUNCH(K, C)                                                                        \
+        // periodic z that the partitioned kernels do not take: Sherman-Morrison, three sweeps; two checkpoint
+        // tables [ceil(nz / CB)][TH] in shared memory (at most 256 checkpoints x 32 threads, or 64 x 64)
+#define PP_Z_LAUNCH(C, T)                                                                        \
         do {                                                                                     \
-            if (int rc = set_smem(K<C>, ds)) return rc;                                          \
-            K<C><<<grid, TH, ds, st>>>(w, zp);                                                   \
+            const size_t ds = 2 * (size_t)((p->nz + C - 1) / C) * T * sizeof(double);            \
+            if (int rc = set_smem(zsolve_cyclic_kernel<C, T>, ds)) return rc;                    \
+            zsolve_cyclic_kernel<C, T><<<(unsigned)((plane + T - 1) / T), T, ds, st>>>(w, zp);   \
         } while (0)
-        if (cb == 16)      PP_Z_LAUNCH(zsolve_cyclic_kernel, 16);
-        else if (cb == 32) PP_Z_LAUNCH(zsolve_cyclic_kernel, 32);
-        else               PP_Z_LAUNCH(zsolve_cyclic_kernel, 64);
+        if (p->nz <= 16 * Z_MAX_CK)      PP_Z_LAUNCH(16, 64);
+        else if (p->nz <= 32 * Z_MAX_CK) PP_Z_LAUNCH(32, 64);
+        else if (p->nz <= 32 * 256)      PP_Z_LAUNCH(32, 32);
+        else                             PP_Z_LAUNCH(64, 32);
 #undef PP_Z_LAUNCH
     }
     return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;

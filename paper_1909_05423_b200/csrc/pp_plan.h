@@ -48,7 +48,7 @@ struct pp_plan {
 
 namespace pp {
 
-// Opt a kernel in to more than 48 KB of dynamic shared memory -- once per (device, kernel, size): pp_solve
+// Opt a kernel in to more than 48 KB of dynamic shared memory -- once per (device, kernel) and size reached: pp_solve
 // itself then only launches (no attribute call on the launch path of the small, latency-bound grids, and
 // nothing but launches inside a stream capture after the first solve).  Defined in pp_api.cu.
 int set_smem_once(const void *kernel, size_t smem);

@@ -90,6 +90,7 @@ __device__ __forceinline__ void zp_minors(double d0, double dint, double dlast, 
 struct ZHier {
     int nK;                  // super-segments per line
     double *HF, *HL;         // [nK][plane]
+    int periodic;            // periodic z: no super-segment is an end of the line, the chain of super-segments closes
 };
 
 template <int R, int MODE, bool CYC = false>
@@ -119,8 +120,8 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
     const bool live = e < plane;
     const bool pin = !live || (p.singular && e == 0);       // pinned line: computed with a placeholder, never stored
     const int K = (MODE == 0) ? 0 : (int)blockIdx.y;         // super-segment of this CTA
-    const bool top_end = !cyc && ((MODE == 0) || K == 0);          // the CTA's rows start at the line's first row
-    const bool bot_end = !cyc && ((MODE == 0) || K == h.nK - 1);   // ... end at its last row
+    const bool top_end = !cyc && ((MODE == 0) || (K == 0 && !h.periodic));          // the CTA's rows start at the line's first row
+    const bool bot_end = !cyc && ((MODE == 0) || (K == h.nK - 1 && !h.periodic));   // ... end at its last row
     const bool mirror = bot_end && (S > 1) && (j == S - 1);   // line's last segment: rows held in reverse order
     const int c = ((j == 0 && top_end) || (j == S - 1 && bot_end)) ? 0 : 1;   // first (and mirrored last) / interior block
     // row i of the segment lives at row0 + i * step (the mirrored segment walks upwards)
@@ -135,8 +136,8 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
     if (j <= jfac && !pin) s = __ldg(p.sx + (int)(e % p.nx)) + __ldg(p.sy + (int)(e / p.nx));
     double ext0 = 0.0, ext1 = 0.0;                            // x just above the CTA's first row / below its last
     if (MODE == 2 && live) {
-        if (j == 0 && !top_end) ext0 = h.HL[(size_t)(K - 1) * plane + e];
-        if (j == S - 1 && !bot_end) ext1 = h.HF[(size_t)(K + 1) * plane + e];
+        if (j == 0 && !top_end) ext0 = h.HL[(size_t)((K > 0) ? K - 1 : h.nK - 1) * plane + e];
+        if (j == S - 1 && !bot_end) ext1 = h.HF[(size_t)((K + 1 < h.nK) ? K + 1 : 0) * plane + e];
     }
     double y[R];
 #pragma unroll
@@ -452,10 +453,130 @@ zsolve_hier_interface_kernel(ZParams p, ZHier h, int rows, double *SC, double *S
     }
 }
 
-// The singular (0,0) line of a long Neumann-z problem (R11), by one CTA of
+// Periodic z on two levels: every super-segment is an interior block and the chain of nK interfaces closes on
+// itself.  Same treatment as inside the CTA (zsolve_part_kernel, CYC): the open chain is factored and solved for
+// the right-hand side and for the two unit vectors of the wrap-around couplings (z1 = chain^-1 e(row a_0),
+// z2 = chain^-1 e(row c_{nK-1})), and a 2x2 closure gives the wrapped unknowns -- an exact cyclic solve, in place
+// of Sherman-Morrison's second sweep over the whole line.
+// In / out as zsolve_hier_interface_kernel, with K + 1 and K - 1 taken modulo nK.  W: [6][nK][plane] scratch.
+__global__ void __launch_bounds__(64)
+zsolve_hier_interface_cyclic_kernel(ZParams p, ZHier h, int rows, double *W) {
+    const size_t plane = (size_t)p.nx * p.ny;
+    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= plane || (p.singular && e == 0)) return;
+    const double s = p.sx[e % p.nx] + p.sy[e / p.nx];
+    const double bint = -2.0 + s;
+    double im = 1.0, ic = bint, prod = 1.0;
+    for (int k0 = 0; k0 + 1 < rows; k0 += 31) {       // 31 steps per renormalisation: |minor| <= bmax^32 (zpart_range_ok)
+#pragma unroll
+        for (int k = 1; k <= 31; ++k) {
+            if (k0 + k < rows) {
+                const double in = fma(bint, ic, -im);
+                im = ic; ic = in;
+            }
+        }
+        const double ri = fast_rcp(ic);
+        prod *= ri;
+        im *= ri; ic = 1.0;
+    }
+    const double a1 = im, b1 = -prod;
+    const int nK = h.nK;
+    const size_t slab = (size_t)nK * plane;
+    double *SC = W + e, *SA = SC + slab, *Z1C = SA + slab, *Z1A = Z1C + slab, *Z2C = Z1A + slab, *Z2A = Z2C + slab;
+    double *HF = h.HF + e, *HL = h.HL + e;
+    const double k1 = fma(b1, b1, -a1 * a1);
+    constexpr int CH = 8;                 // values are fetched CH steps at a time (the loops are latency bound)
+    {
+        double N = a1, M = 1.0, pa = 0.0, pa1 = 0.0;
+        for (int J0 = 0; J0 < nK; J0 += CH) {
+            double yl[CH], yf[CH];
+#pragma unroll
+            for (int i = 0; i < CH; ++i) {
+                const int J = min(J0 + i, nK - 1);
+                yl[i] = HL[(size_t)J * plane];
+                yf[i] = HF[(size_t)((J + 1 < nK) ? J + 1 : 0) * plane];
+            }
+#pragma unroll
+            for (int i = 0; i < CH; ++i) {
+                const int J = J0 + i;
+                if (J < nK) {
+                    const int JF = (J + 1 < nK) ? J + 1 : 0;
+                    const double vL = (J == 0) ? 0.0 : b1, wF = (J == nK - 1) ? 0.0 : b1;
+                    const double r = fast_rcp(fma(-a1, N, M));
+                    const double D = M * r, AD = N * r;
+                    const double Ya = fma(-vL, pa, yl[i]);
+                    const double t = fma(-a1, Ya, yf[i]);
+                    pa = fma(-AD, t, Ya);
+                    const double Ya1 = fma(-vL, pa1, (J == 0) ? 1.0 : 0.0);
+                    const double t1 = -a1 * Ya1;
+                    pa1 = fma(-AD, t1, Ya1);
+                    HF[(size_t)JF * plane] = D * t;                 // pc_J
+                    HL[(size_t)J * plane] = pa;                     // pa_J
+                    SC[(size_t)J * plane] = D * wF;
+                    SA[(size_t)J * plane] = -AD * wF;
+                    Z1C[(size_t)J * plane] = D * t1;
+                    Z1A[(size_t)J * plane] = pa1;
+                    Z2C[(size_t)J * plane] = (J == nK - 1) ? D : 0.0;
+                    Z2A[(size_t)J * plane] = (J == nK - 1) ? -AD : 0.0;
+                    const double Nn = fma(k1, N, a1 * M), Mn = fma(-a1, N, M);
+                    const double nrm = fast_rcp(fabs(Mn) > fabs(Nn) ? Mn : Nn);
+                    N = Nn * nrm;
+                    M = Mn * nrm;
+                }
+            }
+        }
+    }
+    double z1a_last = 0.0, z2a_last = 0.0, z1c_0 = 0.0, z2c_0 = 0.0, x0a = 0.0, x0c = 0.0;
+    {
+        double cn = 0.0, c1 = 0.0, c2 = 0.0;
+        for (int J0 = nK - 1; J0 >= 0; J0 -= CH) {
+            double sc[CH], sa[CH], pc[CH], pv[CH], u1c[CH], u1a[CH], u2c[CH], u2a[CH];
+#pragma unroll
+            for (int i = 0; i < CH; ++i) {
+                const int J = max(J0 - i, 0);
+                sc[i] = SC[(size_t)J * plane];
+                sa[i] = SA[(size_t)J * plane];
+                pc[i] = HF[(size_t)((J + 1 < nK) ? J + 1 : 0) * plane];
+                pv[i] = HL[(size_t)J * plane];
+                u1c[i] = Z1C[(size_t)J * plane]; u1a[i] = Z1A[(size_t)J * plane];
+                u2c[i] = Z2C[(size_t)J * plane]; u2a[i] = Z2A[(size_t)J * plane];
+            }
+#pragma unroll
+            for (int i = 0; i < CH; ++i) {
+                const int J = J0 - i;
+                if (J >= 0) {
+                    const int JF = (J + 1 < nK) ? J + 1 : 0;
+                    const double av = fma(-sa[i], cn, pv[i]), a1v = fma(-sa[i], c1, u1a[i]), a2v = fma(-sa[i], c2, u2a[i]);
+                    cn = fma(-sc[i], cn, pc[i]);
+                    c1 = fma(-sc[i], c1, u1c[i]);
+                    c2 = fma(-sc[i], c2, u2c[i]);
+                    HF[(size_t)JF * plane] = cn;                    // open-chain c_J
+                    HL[(size_t)J * plane] = av;                     // open-chain a_J
+                    Z1C[(size_t)J * plane] = c1; Z1A[(size_t)J * plane] = a1v;
+                    Z2C[(size_t)J * plane] = c2; Z2A[(size_t)J * plane] = a2v;
+                    if (J == nK - 1) { z1a_last = a1v; z2a_last = a2v; x0a = av; }
+                    if (J == 0) { z1c_0 = c1; z2c_0 = c2; x0c = cn; }
+                }
+            }
+        }
+    }
+    // closure:  K (a_{nK-1}, c_0)^T = (x0a, x0c)^T,  K = [1 + b1 z1a_{nK-1}, b1 z2a_{nK-1}; b1 z1c_0, 1 + b1 z2c_0];
+    //           x = x0 - (b1 a_{nK-1}) z1 - (b1 c_0) z2
+    const double k11 = fma(b1, z1a_last, 1.0), k12 = b1 * z2a_last, k21 = b1 * z1c_0, k22 = fma(b1, z2c_0, 1.0);
+    const double rdet = b1 / fma(k11, k22, -k12 * k21);
+    const double ba = (k22 * x0a - k12 * x0c) * rdet, bg = (k11 * x0c - k21 * x0a) * rdet;
+    for (int J = 0; J < nK; ++J) {
+        const int JF = (J + 1 < nK) ? J + 1 : 0;
+        HF[(size_t)JF * plane] = fma(-ba, Z1C[(size_t)J * plane], fma(-bg, Z2C[(size_t)J * plane], HF[(size_t)JF * plane]));
+        HL[(size_t)J * plane] = fma(-ba, Z1A[(size_t)J * plane], fma(-bg, Z2A[(size_t)J * plane], HL[(size_t)J * plane]));
+    }
+}
+
+// The singular (0,0) line of a long Neumann- or periodic-z problem (R11), by one CTA of
 // 1024 threads: the same two running sums as zero_mode_line, each thread holding its contiguous
 // chunk of at most 16 rows in registers (nz <= 16384), chunk totals combined by block-wide scans.
-//   r <- (r - mean r) scale;  x_0 = 0;  d_k = -sum_{m >= k} r_m;  x_k = sum_{1 <= m <= k} d_m;  x <- x - mean x
+//   r <- (r - mean r) scale;  x_0 = 0;  d_k = -sum_{m >= k} r_m  (periodic: d_1 + sum_{1 <= m < k} r_m);
+//   x_k = sum_{1 <= m <= k} d_m;  x <- x - mean x
 __device__ __forceinline__ double zp_block_excl_scan(double v, double *red, double &total) {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const double wex = warp_excl_scan(v, lane);
@@ -470,7 +591,7 @@ __device__ __forceinline__ double zp_block_excl_scan(double v, double *red, doub
 }
 
 __global__ void __launch_bounds__(1024, 1)
-zero_mode_long_kernel(double *col, size_t plane, int nz, double scale, int pin_plane0) {
+zero_mode_long_kernel(double *col, size_t plane, int nz, double scale, int pin_plane0, int periodic) {
     __shared__ double red[32];
     constexpr int C = 16;
     const int c = (nz + (int)blockDim.x - 1) / (int)blockDim.x;        // <= C
@@ -495,13 +616,35 @@ zero_mode_long_kernel(double *col, size_t plane, int nz, double scale, int pin_p
     double all;
     double run = zp_block_excl_scan(own, red, all);
     double dsum = 0.0;
+    if (!periodic) {
 #pragma unroll
-    for (int i = 0; i < C; ++i) {
-        const bool in = i < c && k0 + i < k1 && k0 + i >= 1;
-        const double r = v[i];
-        v[i] = in ? -(all - run) : 0.0;                               // d_k
-        run += r;
-        dsum += v[i];
+        for (int i = 0; i < C; ++i) {
+            const bool in = i < c && k0 + i < k1 && k0 + i >= 1;
+            const double r = v[i];
+            v[i] = in ? -(all - run) : 0.0;                           // Neumann: d_k = -sum_{m >= k} r_m
+            run += r;
+            dsum += v[i];
+        }
+    } else {
+        // periodic: d_k = d_1 + S_{k-1}, S_j = sum_{1 <= m <= j} r_m, and x_n = x_0 = 0 fixes d_1 = -(sum_k S_{k-1} + S_{n-1}) / n
+        double ssum = 0.0;
+#pragma unroll
+        for (int i = 0; i < C; ++i) {
+            const bool in = i < c && k0 + i < k1 && k0 + i >= 1;
+            const double r = v[i];
+            v[i] = in ? run : 0.0;                                    // S_{k-1}
+            run += r;
+            ssum += v[i];
+        }
+        double stot;
+        zp_block_excl_scan(ssum, red, stot);
+        const double d1 = -(stot + all) / nz;
+#pragma unroll
+        for (int i = 0; i < C; ++i) {
+            const bool in = i < c && k0 + i < k1 && k0 + i >= 1;
+            v[i] = in ? v[i] + d1 : 0.0;
+            dsum += v[i];
+        }
     }
     double dummy;
     double x = zp_block_excl_scan(dsum, red, dummy);

@@ -325,13 +325,15 @@ zsolve_thomas_kernel(double *w, ZParams p) {
 // Periodic in z: Sherman-Morrison, "two solves".  With gamma = -b:
 //   T' = T - w v^T,  w = (gamma,0,..,0,1)^T, v = (1,0,..,0,1/gamma)^T,  b'_0 = 2b, b'_{n-1} = b + 1/b
 //   x = T'^-1 r,  q = T'^-1 w,  u = x - q (v.x)/(1 + v.q).
-// q depends only on the mode, so it is never stored: it is recomputed next to the pivots.
+// q depends only on the mode, so it is never stored: it is recomputed next to the pivots, from checkpoints
+// kept every CB rows in shared memory.
 // Sweep 1 forward (x'), sweep 2 backward (x, and q to get the scalar), sweep 3 backward (u).
-template <int CB>
-__global__ void __launch_bounds__(PP_Z_THREADS, PP_Z_MINB)
+template <int CB, int TH>
+__global__ void __launch_bounds__(TH, PP_Z_MINB)
 zsolve_cyclic_kernel(double *w, ZParams p) {
+    extern __shared__ double ck[];                 // [2][nblk][TH] checkpoints of the pivot and of the q sweep
     const size_t plane = (size_t)p.nx * p.ny;
-    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t e = (size_t)blockIdx.x * TH + threadIdx.x;
     const bool live = e < plane;
     const int ix = live ? (int)(e % p.nx) : 0, j = live ? (int)(e / p.nx) : 0;
     const bool pin = !live || (p.singular && e == 0);
@@ -344,12 +346,13 @@ zsolve_cyclic_kernel(double *w, ZParams p) {
     const double scale = p.scale;
     double *col = w + (live ? e : 0);
     const ZPolicy pol;
-    double ckg[Z_MAX_CK], ckq[Z_MAX_CK];
+    const int nblk = (nz + CB - 1) / CB;
+    double *ckg = ck + threadIdx.x, *ckq = ckg + (size_t)nblk * TH;     // entry of block i at [i * TH]
 
     double g = 0.0, xp = 0.0, qp = 0.0;
     for (int k0 = 0; k0 < nz; k0 += CB) {
-        ckg[k0 / CB] = g;
-        ckq[k0 / CB] = qp;
+        ckg[(k0 / CB) * TH] = g;
+        ckq[(k0 / CB) * TH] = qp;
         double r[CB];
 #pragma unroll
         for (int i = 0; i < CB; ++i) r[i] = (k0 + i < nz) ? ld_hint(col + (size_t)(k0 + i) * plane, pol.first) : 0.0;
@@ -373,7 +376,7 @@ zsolve_cyclic_kernel(double *w, ZParams p) {
         if (sweep == 1 && !pin) col[(size_t)(nz - 1) * plane] = xlast - fac * qlast;
         for (int k0 = ((nz - 1) / CB) * CB; k0 >= 0; k0 -= CB) {
             double gl[CB], ql[CB], r[CB];
-            double gg = ckg[k0 / CB], qq = ckq[k0 / CB];
+            double gg = ckg[(k0 / CB) * TH], qq = ckq[(k0 / CB) * TH];
 #pragma unroll
             for (int i = 0; i < CB; ++i) r[i] = (k0 + i < nz - 1) ? ld_hint(col + (size_t)(k0 + i) * plane, sweep == 0 ? pol.last : pol.first) : 0.0;
 #pragma unroll

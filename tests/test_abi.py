@@ -54,9 +54,8 @@ def test_validation_without_device():
     assert pp.pp_plan_create(32, 112, 32, 0.1, 0.1, 0.1, 0, 0, 0)[0] == 2     # 7*2^4
     assert pp.pp_plan_create(32, 4096, 32, 0.1, 0.1, 0.1, 0, 0, 0)[0] == 2    # too long
     assert pp.pp_plan_create(32, 32, 1, 0.1, 0.1, 0.1, 0, 0, 0)[0] == 2       # nz < 2
-    assert pp.pp_plan_create(32, 32, 8192, 0.1, 0.1, 0.1, 0, 0, 0)[0] == 2    # long lines need non-periodic z
-    assert pp.pp_plan_create(32, 32, 8192 + 64, 0.1, 0.1, 0.1, 0, 0, 1)[0] == 2   # ... and nz = 256 m
-    assert pp.pp_plan_create(32, 32, 32768, 0.1, 0.1, 0.1, 0, 0, 1)[0] == 2   # ... up to 16384
+    assert pp.pp_plan_create(32, 32, 16384 + 1, 0.1, 0.1, 0.1, 0, 0, 0)[0] == 2   # lines up to 16384 rows
+    assert pp.pp_plan_create(32, 32, 32768, 0.1, 0.1, 0.1, 0, 0, 1)[0] == 2
     assert pp.binding.pp_plan_set_z_algorithm(0, 1) == 5                      # NULL plan
     assert pp.binding.pp_plan_set_xy_fusion(0, 1) == 5
     assert pp.binding.pp_plan_launches_per_solve(0) == 0
@@ -92,7 +91,7 @@ def test_product_path_does_not_import_the_oracle():
 
 def test_size_rules_host_side():
     """pp_size_supported needs no device: 2^k in [4, 2048], 3*2^k in [48, 1536], 5*2^k in [80, 1280];
-    nz in [2, 4096], or 256 m <= 16384 with non-periodic z."""
+    nz in [2, 16384], any boundary condition in z."""
     import paper_1909_05423_b200 as pp
     ok = pp.binding.pp_size_supported
     good = [4, 8, 512, 2048, 48, 96, 192, 384, 768, 1536, 80, 160, 320, 640, 1280]
@@ -103,7 +102,8 @@ def test_size_rules_host_side():
         assert not ok(n, 64, 32, 1) and not ok(64, n, 32, 0), n
     assert ok(64, 64, 2, 0) and ok(64, 64, 4096, 0) and not ok(64, 64, 1, 0)
     assert ok(64, 64, 16384, 1) and ok(48, 48, 8192, 2)
-    assert not ok(64, 64, 16384, 0)              # long lines: non-periodic z only
-    assert not ok(64, 64, 8192 + 32, 1)          # ... in multiples of 256
-    assert not ok(64, 64, 32768, 1)              # ... up to 16384
+    for bcz in (0, 1, 2):                        # every nz in [2, 16384] with every boundary condition in z
+        for nz in (2, 3, 100, 4096, 4097, 5000, 8200, 8192 + 32, 16383, 16384):
+            assert ok(64, 64, nz, bcz), (nz, bcz)
+        assert not ok(64, 64, 16385, bcz) and not ok(64, 64, 32768, bcz)
     assert not ok(64, 64, 64, 7)                 # unknown boundary condition

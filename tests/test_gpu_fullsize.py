@@ -14,7 +14,7 @@ import pytest
 from oracle import poisson_oracle as po
 from paper_1909_05423_b200 import workloads as wl
 from gpu_util import TOL, rel_err
-from oracle_blocked import oracle_solve_blocked
+from oracle_blocked import oracle_solve_blocked, rel_err_blocked
 from stencil_sampling import gather_torch, neighbour_table, sample_indices
 
 pytestmark = pytest.mark.gpu

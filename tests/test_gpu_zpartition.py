@@ -78,7 +78,7 @@ def test_extreme_anisotropy_falls_back_to_the_sweep():
 
 def test_partition_refused_where_it_does_not_apply():
     import paper_1909_05423_b200 as pp
-    for nz, combo in ((48, "PPN"), (768, "PPP"), (100, "DDD")):
+    for nz, combo in ((48, "PPN"), (800, "PPP"), (100, "DDD")):
         plan = pp.Plan(8, 8, nz, 0.1, 0.1, 0.1, combo)
         with pytest.raises(pp.PittPackError):
             plan.set_z_algorithm("partition")
@@ -89,10 +89,11 @@ def test_partition_refused_where_it_does_not_apply():
 
 # ---------------------------------------------------------------- long lines: two-level partition
 @pytest.mark.parametrize("nz", [512 + 256, 1280, 2304, 4096])
-@pytest.mark.parametrize("combo", ["PPN", "NND", "DDD", "NNN"])
+@pytest.mark.parametrize("combo", ["PPN", "NND", "DDD", "NNN", "PPP", "NNP", "DNP"])
 def test_two_level_partition_matches_oracle(nz, combo):
     """nz = 256 m that no single CTA holds: super-segments of 256 rows coupled by the interface
-    kernel.  At nz <= 4096 the two-sweep kernel solves the same systems: both must match the oracle."""
+    kernel (periodic z: the chain of super-segments closes on itself).  The two-sweep kernel solves the
+    same systems: both must match the oracle."""
     bc = wl.parse_bc(combo)
     shape = (nz, 4, 24 if False else 16)
     h = (1.0 / 16, 1.0 / 4, 1.0 / 8)
@@ -103,7 +104,7 @@ def test_two_level_partition_matches_oracle(nz, combo):
         assert e <= TOL, (alg, nz, combo, e)
 
 
-@pytest.mark.parametrize("combo", ["PPD", "PPN"])
+@pytest.mark.parametrize("combo", ["PPD", "PPN", "PPP", "NNP"])
 def test_paper_pencil_shape(combo):
     """64 x 64 x 16384, the paper's per-GPU weak-scaling load: beyond the two-sweep
     kernel's range, solved by the two-level partition only."""
@@ -127,12 +128,27 @@ def test_paper_pencil_48():
     assert e <= TOL, e
 
 
+@pytest.mark.parametrize("nz", [5000, 8200, 4097, 16383])
+@pytest.mark.parametrize("combo", ["PPN", "NND", "PPP"])
+def test_long_lines_of_any_length(nz, combo):
+    """nz beyond 4096 that is not a multiple of 256 (the two-level partition does not take it): the two-sweep
+    kernels with their checkpoint tables in shared memory.  Ground truth: the oracle with a long-double z solve."""
+    bc = wl.parse_bc(combo)
+    shape, h = (nz, 8, 16), (1.0 / 16, 1.0 / 8, 1.0 / 16)
+    f = wl.random_normal(shape, 3000 + nz, zero_mean=all(b in (0, 1) for b in bc))
+    ref = po.solve(f, h, bc, zdtype=np.longdouble)
+    e = rel_err(gpu_solve(f, h, bc), ref)
+    assert e <= TOL, (nz, combo, e)
+
+
 def test_long_line_limits():
     import paper_1909_05423_b200 as pp
-    for nz, combo, ok in ((8192, "PPN", True), (8192, "PPP", False), (8192 + 128, "PPN", False), (32768, "PPD", False)):
+    for nz, combo, ok in ((8192, "PPN", True), (8192, "PPP", True), (8192 + 128, "PPN", True), (16384, "NNP", True),
+                          (16385, "PPN", False), (32768, "PPD", False)):
         st, h = pp.binding.pp_plan_create(8, 8, nz, 0.1, 0.1, 0.1, *wl.parse_bc(combo))
         assert (st == 0) == ok, (nz, combo, st)
         if h:
-            if ok:
-                assert pp.binding.pp_plan_set_z_algorithm(h, pp.binding.PP_Z_SWEEP) != 0
+            assert pp.binding.pp_plan_set_z_algorithm(h, pp.binding.PP_Z_SWEEP) == 0      # any nz has a two-sweep path
+            want = 0 if nz % 256 == 0 else 2                                              # two-level: multiples of 256
+            assert pp.binding.pp_plan_set_z_algorithm(h, pp.binding.PP_Z_PARTITION) == want
             pp.binding.pp_plan_destroy(h)
