@@ -10,7 +10,23 @@ int launch_y_fwd(double *w, int nxh, int nz, int bc, int complex_cols, const dou
                  const YRows *rows, cudaStream_t st) {
     using Y = YCfg<N>;
     const dim3 grid((unsigned)((nxh + Y::T - 1) / Y::T), (unsigned)nz);
-    if (rows) {
+    if (!rows && YStaged<N>::ON) {
+        // persistent staged kernel: one wave of resident CTAs walks over all tiles
+        using S = YStaged<N>;
+        auto k = ypass_staged_kernel<N, true>;
+        if (int rc = set_smem(k, S::SMEM)) return rc;
+        static int sms = 0;
+        if (!sms) {
+            int dev = 0;
+            if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+                cudaGetLastError();
+                sms = 0;
+                return PP_ERR_CUDA;
+            }
+        }
+        const long long total = (long long)grid.x * grid.y, resident = (long long)sms * S::PER_SM;
+        k<<<(unsigned)(total < resident ? total : resident), Y::THREADS, S::SMEM, st>>>((double2 *)w, nxh, nz, bc, complex_cols, tw, ptw);
+    } else if (rows) {
         auto k = ypass_fwd_slab_kernel<N>;
         if (int rc = set_smem(k, Y::SMEM)) return rc;
         k<<<grid, Y::THREADS, Y::SMEM, st>>>((double2 *)w, nxh, bc, complex_cols, tw, ptw, *rows);

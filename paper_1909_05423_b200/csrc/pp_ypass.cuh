@@ -59,7 +59,7 @@ struct SyncCta {
 #define PP_Y_T_1024 4     // ... for N in (512, 1024]
 #endif
 #ifndef PP_Y_T_2048
-#define PP_Y_T_2048 4     // ... for N > 1024
+#define PP_Y_T_2048 2     // ... for N > 1024 (32-byte row segments: two resident CTAs per SM beat one with 64-byte ones, measured)
 #endif
 #ifndef PP_Y_MINB
 #define PP_Y_MINB 2       // __launch_bounds__ min CTAs per SM (caps registers) for CTAs of <= 512 threads
@@ -103,13 +103,84 @@ struct YRows {
     }
 };
 
+// ---- staged tiles (persistent kernel, north_star item 3 "staged tiles") ---------------------------------------
+// A resident CTA walks over tiles and copies its NEXT tile from global into a second shared-memory buffer with
+// asynchronous 16-byte copies (cp.async / LDGSTS: no registers, no scoreboard wait) while it transforms the current
+// one -- the load latency that the plain kernels expose once per tile (ncu: long-scoreboard stalls, one or two
+// resident CTAs per SM at N >= 1024) is hidden behind a whole tile of arithmetic.  The copy applies the pass's row
+// permutation on the way, so the staged tile is read back in natural order: rows t, t+1 of
+// a quarter-warp are adjacent, conflict-free without padding.
+__device__ __forceinline__ void cp_async16(double2 *smem_dst, const double2 *gmem_src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+struct NoHook {
+    __device__ __forceinline__ void operator()() const {}
+};
+
+#ifndef PP_Y_STAGED_MIN
+#define PP_Y_STAGED_MIN 4096      // y pass: staged persistent kernel from this length on (4096: never)
+#endif
+template <int N>
+struct YStaged {
+    static constexpr bool ON = (N >= PP_Y_STAGED_MIN);
+    static constexpr size_t IN_BYTES = size_t(YCfg<N>::T) * N * sizeof(double2);
+    static constexpr size_t SMEM = YCfg<N>::SMEM + IN_BYTES;
+    static constexpr int PER_SM_SMEM = int((227 * 1024) / (SMEM + 1024));
+    static constexpr int PER_SM_THREADS = 2048 / YCfg<N>::THREADS;
+    static constexpr int REGS = (YCfg<N>::E <= 12 && YCfg<N>::E != 12) ? 64 : 128;
+    static constexpr int PER_SM_REGS = 65536 / (REGS * YCfg<N>::THREADS);
+    static constexpr int PER_SM0 = PER_SM_SMEM < PER_SM_THREADS ? PER_SM_SMEM : PER_SM_THREADS;
+    static constexpr int PER_SM = (PER_SM0 < PER_SM_REGS ? PER_SM0 : PER_SM_REGS) > 0 ? (PER_SM0 < PER_SM_REGS ? PER_SM0 : PER_SM_REGS) : 1;
+};
+
+// copies of one tile of the forward pass into `stage`: position i <- the row the transform wants at input i
+template <int N>
+__device__ __forceinline__ void yfwd_stage_issue(const double2 *w, int nxh, int bc, int bx, int z, double2 *stage) {
+    using C = typename YCfg<N>::F;
+    constexpr int E = C::E, P = C::P, T = YCfg<N>::T, H = N / 2;
+    const int c = threadIdx.x % T, t = threadIdx.x / T;
+    const int cp = bx * T + c;
+    const double2 *base = w + (size_t)z * N * nxh + (cp < nxh ? cp : 0);
+#pragma unroll
+    for (int q = 0; q < E; ++q) {
+        const int i = t + q * P;
+        int row = i;
+        if (bc == BC_N) row = (i < H) ? 2 * i : 2 * (N - 1 - i) + 1;
+        else if (bc == BC_D) row = (i < H) ? N - 1 - 2 * i : 2 * i - N;
+        cp_async16(stage + i * T + c, base + row * nxh);
+    }
+    cp_async_commit();
+}
+// ... of the inverse pass: rows in natural order
+template <int N>
+__device__ __forceinline__ void yinv_stage_issue(const double2 *w, int nxh, int bx, int z, double2 *stage) {
+    using C = typename YCfg<N>::F;
+    constexpr int E = C::E, P = C::P, T = YCfg<N>::T;
+    const int c = threadIdx.x % T, t = threadIdx.x / T;
+    const int cp = bx * T + c;
+    const double2 *base = w + (size_t)z * N * nxh + (cp < nxh ? cp : 0);
+#pragma unroll
+    for (int q = 0; q < E; ++q) {
+        const int j = t + q * P;
+        cp_async16(stage + j * T + c, base + j * nxh);
+    }
+    cp_async_commit();
+}
+
 // One CTA-wide tile of the forward y pass: column tile bx (T double2 columns) of plane z, all N rows
 // (blockDim.x == YCfg<N>::THREADS).  `smem` holds YCfg<N>::SMEM bytes.  LDCG: read with
 // ld.global.cg -- for the fused x+y kernel, whose input was just written by other SMs.
-template <int N, bool LDCG, bool SLAB = false>
+// STAGED: the tile's input was copied to `stage` by yfwd_stage_issue; `after_load` runs when every thread has its
+// input in registers (the staged kernel puts a barrier and the next tile's copies there).
+template <int N, bool LDCG, bool SLAB = false, bool STAGED = false, class Hook = NoHook>
 __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int complex_cols,
                                           const double2 *__restrict__ tw, const double2 *__restrict__ ptw,
-                                          int bx, int z, double2 *smem, const YRows *rows = nullptr) {
+                                          int bx, int z, double2 *smem, const YRows *rows = nullptr,
+                                          const double2 *stage = nullptr, const Hook &after_load = Hook()) {
     using C = typename YCfg<N>::F;
     constexpr int E = C::E, P = C::P, T = YCfg<N>::T, H = N / 2;
     const int c = threadIdx.x % T, t = threadIdx.x / T;
@@ -129,7 +200,10 @@ __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int compl
 #pragma unroll
     for (int q = 0; q < E; ++q) {
         const int i = t + q * P;
-        if (bc == BC_P) {
+        if constexpr (STAGED) {
+            v[q] = stage[i * T + c];
+            if (bc == BC_D && i >= H) v[q] = dscale(-1.0, v[q]);
+        } else if (bc == BC_P) {
             v[q] = yld<LDCG>(base + i * ld);
         } else if (bc == BC_N) {
             const int p = (i < H) ? 2 * i : 2 * (N - 1 - i) + 1;
@@ -139,6 +213,7 @@ __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int compl
             else       v[q] = dscale(-1.0, yld<LDCG>(base + (2 * i - N) * ld));
         }
     }
+    after_load();
 
     fft<N, FWD>(v, t, smem, tw, lay, sync);
 
@@ -221,10 +296,11 @@ ypass_fwd_slab_kernel(double2 *w, int nxh, int bc, int complex_cols,
 }
 
 // One CTA-wide tile of the inverse y pass (see yfwd_tile).
-template <int N, bool SLAB = false>
+template <int N, bool SLAB = false, bool STAGED = false, class Hook = NoHook>
 __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int complex_cols,
                                           const double2 *__restrict__ tw, const double2 *__restrict__ ptw,
-                                          int bx, int z, double2 *smem, const YRows *rows = nullptr) {
+                                          int bx, int z, double2 *smem, const YRows *rows = nullptr,
+                                          const double2 *stage = nullptr, const Hook &after_load = Hook()) {
     using C = typename YCfg<N>::F;
     constexpr int E = C::E, P = C::P, T = YCfg<N>::T, H = N / 2;
     const int c = threadIdx.x % T, t = threadIdx.x / T;
@@ -237,7 +313,8 @@ __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int compl
     const bool cplx = complex_cols && cp > 0;
     // where row j of the input comes from: in place, or (slab decomposition) the owner rank's pencil block
     const auto in = [&](int j) -> const double2 * {
-        if constexpr (SLAB) return rows->row(z, j, ld) + (active ? cp : 0);
+        if constexpr (STAGED) return stage + j * T + c;
+        else if constexpr (SLAB) return rows->row(z, j, ld) + (active ? cp : 0);
         else return base + j * ld;
     };
 
@@ -245,6 +322,7 @@ __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int compl
     if (complex_cols && bx > 0) {                          // block-uniform: every column of the tile is complex
 #pragma unroll
         for (int q = 0; q < E; ++q) v[q] = *in((t + q * P));
+        after_load();
     } else {
         // Real pairs: row m and row N-m are needed together, for V_m and for V_{N-m}.  The owner of
         // m in [0, N/2) loads the two rows once, keeps V_m and hands V_{N-m} to its owner through shared
@@ -269,6 +347,7 @@ __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int compl
                 if (m == 0) yh = *in((N - 1 - H));
             }
         }
+        after_load();
         if (!cplx) {
 #pragma unroll
             for (int q = 0; q < E / 2; ++q) {
@@ -337,6 +416,38 @@ ypass_inv_slab_kernel(double2 *w, int nxh, int bc, int complex_cols,
                       const double2 *__restrict__ tw, const double2 *__restrict__ ptw, const __grid_constant__ YRows rows) {
     extern __shared__ double2 smem[];
     yinv_tile<N, true>(w, nxh, bc, complex_cols, tw, ptw, blockIdx.x, blockIdx.y, smem, &rows);
+}
+
+// Persistent staged kernels: CTA b transforms tiles b, b + gridDim.x, ... (tile = column tile bx of plane z, bx
+// fastest: the resident CTAs work on neighbouring row segments of the same planes).  smem: the exchange scratch
+// of the plain kernels, then the staging buffer.
+template <int N, bool FWD_DIR>
+__global__ void __launch_bounds__(YCfg<N>::THREADS, YStaged<N>::PER_SM)
+ypass_staged_kernel(double2 *w, int nxh, int nz, int bc, int complex_cols,
+                    const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
+    extern __shared__ double2 smem[];
+    double2 *stage = smem + YCfg<N>::SMEM / sizeof(double2);
+    constexpr int T = YCfg<N>::T;
+    const int ntx = (nxh + T - 1) / T, total = ntx * nz;
+    // forward: planes from the last to the first (the x pass before it left its last planes in L2)
+    const auto plane_of = [&](int tile) { return FWD_DIR ? nz - 1 - tile / ntx : tile / ntx; };
+    const auto issue = [&](int tile) {
+        if (FWD_DIR) yfwd_stage_issue<N>(w, nxh, bc, tile % ntx, plane_of(tile), stage);
+        else         yinv_stage_issue<N>(w, nxh, tile % ntx, plane_of(tile), stage);
+    };
+    int tile = blockIdx.x;
+    if (tile < total) issue(tile);
+    for (; tile < total; tile += gridDim.x) {
+        cp_async_wait_all();
+        __syncthreads();                           // the staged tile is complete; the previous tile is done with smem
+        const int next = tile + (int)gridDim.x;
+        const auto after_load = [&]() {
+            __syncthreads();                       // every thread has read its part of the staging buffer
+            if (next < total) issue(next);
+        };
+        if (FWD_DIR) yfwd_tile<N, false, false, true>(w, nxh, bc, complex_cols, tw, ptw, tile % ntx, plane_of(tile), smem, nullptr, stage, after_load);
+        else         yinv_tile<N, false, true>(w, nxh, bc, complex_cols, tw, ptw, tile % ntx, plane_of(tile), smem, nullptr, stage, after_load);
+    }
 }
 
 }  // namespace pp
