@@ -147,6 +147,49 @@ __device__ __forceinline__ double2 cmul_const(double2 a, double cr, double ci) {
     return make_double2(fma(a.x, cr, -(a.y * si)), fma(a.x, si, a.y * cr));
 }
 
+// Post-/pre-twiddles of the cosine and sine transforms, w_m = exp(-i pi m / (2N)): thread t needs
+// them at m = t + q P, q = 0 .. E/2 - 1, and w_{t + q P} = w_t exp(-i pi q / (2E)) -- one table load per thread, the
+// other E/2 - 1 by a rotation through a compile-time constant (a table load issued between a tile's stores queues
+// behind them: ncu showed one long-scoreboard wait per coefficient pair).  cos / sin of pi q / (2E) <= pi/4 by
+// their Taylor series, evaluated at compile time.
+__host__ __device__ constexpr double ct_cos(double x) {
+    double sum = 1.0, term = 1.0;
+    for (int k = 1; k <= 12; ++k) { term *= -x * x / double((2 * k - 1) * (2 * k)); sum += term; }
+    return sum;
+}
+__host__ __device__ constexpr double ct_sin(double x) {
+    double sum = x, term = x;
+    for (int k = 1; k <= 12; ++k) { term *= -x * x / double((2 * k) * (2 * k + 1)); sum += term; }
+    return sum;
+}
+template <int E>
+struct PtwSteps {
+    double c[E / 2 > 0 ? E / 2 : 1], s[E / 2 > 0 ? E / 2 : 1];
+    constexpr PtwSteps() : c(), s() {
+        for (int q = 0; q < E / 2; ++q) {
+            c[q] = ct_cos(3.14159265358979323846 * q / (2.0 * E));
+            s[q] = ct_sin(3.14159265358979323846 * q / (2.0 * E));
+        }
+    }
+};
+// w_{t + q P} from w_t (q a compile-time constant after unrolling)
+#ifndef PP_PTW_ROT
+#define PP_PTW_ROT 1
+#endif
+#ifndef PP_HOIST_ZC_MIN_E
+#define PP_HOIST_ZC_MIN_E 16     // partner reads hoisted above the stores only where registers allow (16+ elements per thread: 128-register kernels)
+#endif
+template <int E>
+__device__ __forceinline__ double2 ptw_rot(double2 w0, int q, const double2 *ptw = nullptr, int m = 0) {
+    constexpr PtwSteps<E> st;
+#if !PP_PTW_ROT
+    return __ldg(&ptw[m]);
+#endif
+    if (q == 0) return w0;
+    const double c = st.c[q], sn = -st.s[q];         // exp(-i a) = cos a - i sin a
+    return make_double2(fma(w0.x, c, -(w0.y * sn)), fma(w0.x, sn, w0.y * c));
+}
+
 // in-place 16-point DFT, 16 = 4 x 4: 4-point DFTs over n1 (n = 4 n1 + n0), twiddles W_16^(n0 k1), 4-point DFTs
 // over n0.  The result is left transposed: X_{k1 + 4 k2} sits in x[4 k1 + k2] -- read it through bfly16_at.
 __host__ __device__ constexpr int bfly16_at(int k) { return 4 * (k & 3) + (k >> 2); }

@@ -57,7 +57,9 @@ struct XCfg {
     static constexpr int P = F::P;
     static constexpr int T = (256 / P) > 0 ? (256 / P) : 1;   // transforms (row pairs) per CTA; <= 4 when P >= 64
     static constexpr int THREADS = T * P;
-    static constexpr int MINB = (E <= 12) ? PP_X_MINB : 2;    // 16 or 20 elements per thread need more than 64 registers
+    // 8 elements per thread fit 64 registers (four CTAs per SM); 12 need about 80 (three CTAs: at 64 the 3 * 2^k
+    // passes spilled up to 300 bytes per thread), 16 or 20 more than that
+    static constexpr int MINB = (E <= 8) ? PP_X_MINB : ((E == 12) ? 3 : 2);
     static constexpr size_t SMEM = size_t(T) * F::SMEM_ELEMS * sizeof(double2);
 };
 
@@ -107,18 +109,24 @@ __device__ __forceinline__ void xfwd_tile(const double *in, double *out, long lo
     for (int q = E / 2; q < E; ++q) s[lay(t + q * P)] = v[q];
     sync();
     if (active) {
+        // the partners first, all in flight together, and one post-twiddle per thread (ptw_rot): loads issued
+        // between the stores below queue behind them
+        double2 zcs[E / 2];
+        const double2 w0 = (bc != BC_P) ? __ldg(&ptw[t]) : make_double2(1.0, 0.0);
+#pragma unroll
+        for (int q = 0; q < E / 2; ++q) if (E >= PP_HOIST_ZC_MIN_E) zcs[q] = s[lay(neg_mod<N>(t + q * P))];
 #pragma unroll
         for (int q = 0; q < E / 2; ++q) {
             const int m = t + q * P;                       // 0 <= m < N/2
             const double2 zm = v[q];
-            const double2 zc = s[lay(neg_mod<N>(m))];
+            const double2 zc = (E >= PP_HOIST_ZC_MIN_E) ? zcs[q] : s[lay(neg_mod<N>(m))];
             if (m == 0) {
                 const double2 zh = v[E / 2];               // thread 0 also holds Z_{N/2}
                 if (bc == BC_P) {
                     *reinterpret_cast<double2 *>(oa) = make_double2(zm.x, zh.x);
                     *reinterpret_cast<double2 *>(ob) = make_double2(zm.y, zh.y);
                 } else {
-                    const double c4 = ptw[H].x;            // cos(pi/4)
+                    constexpr double c4 = 0.70710678118654752440;   // cos(pi/4) = Re w_{N/2}
                     if (bc == BC_N) {
                         oa[0] = zm.x; ob[0] = zm.y;
                         oa[H] = c4 * zh.x; ob[H] = c4 * zh.y;
@@ -135,7 +143,7 @@ __device__ __forceinline__ void xfwd_tile(const double *in, double *out, long lo
                     *reinterpret_cast<double2 *>(oa + 2 * m) = A;
                     *reinterpret_cast<double2 *>(ob + 2 * m) = B;
                 } else {
-                    const double2 w = __ldg(&ptw[m]);
+                    const double2 w = ptw_rot<E>(w0, q, ptw, m);
                     const double2 ca = cmul(w, A), cb = cmul(w, B);
                     if (bc == BC_N) {
                         oa[m] = ca.x;      ob[m] = cb.x;
@@ -213,6 +221,7 @@ __device__ __forceinline__ void xinv_tile(const double *in, double *out, long lo
         // Packed rows: Y = Ya + i Yb, so Y_m - i Y_{N-m} = (ya + ybp) + i (yb - yap).
         // (all loads first, so that they are in flight together; then the arithmetic)
         double la[E / 2], lb[E / 2], lap[E / 2], lbp[E / 2], ha = 0.0, hb = 0.0;
+        const double2 w0 = __ldg(&ptw[t]);                 // the other pre-twiddles by rotation (ptw_rot)
 #pragma unroll
         for (int q = 0; q < E / 2; ++q) {
             const int m = t + q * P;
@@ -230,13 +239,15 @@ __device__ __forceinline__ void xinv_tile(const double *in, double *out, long lo
             const int m = t + q * P;
             const double s1 = (bc == BC_N) ? 1.0 : sgn_of(m);           // Dirichlet: Y'_m = (-1)^m S_{N-1-m}
             const double ya = s1 * la[q], yb = s1 * lb[q], yap = s1 * lap[q], ybp = s1 * lbp[q];
-            const double2 w = __ldg(&ptw[m]);
+            const double2 w = ptw_rot<E>(w0, q, ptw, m);
             v[q] = cmul(cconj(w), make_double2(ya + ybp, yb - yap));
             if (m > 0) {
                 s[lay(N - m)] = cmul(make_double2(-w.y, w.x), make_double2(yap + yb, ybp - ya));   // i w_m (...)
             } else {
                 const double sh = (bc == BC_N) ? 1.0 : sgn_of(H);
-                s[lay(H)] = cmul(cconj(__ldg(&ptw[H])), make_double2(sh * (ha + hb), sh * (hb - ha)));
+                constexpr double c4 = 0.70710678118654752440;              // conj(w_{N/2}) = c4 (1 + i)
+                const double hr = sh * (ha + hb), hi = sh * (hb - ha);
+                s[lay(H)] = make_double2(c4 * (hr - hi), c4 * (hr + hi));
             }
         }
     }

@@ -233,18 +233,24 @@ __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int compl
         for (int q = 0; q < E; ++q) *out((t + q * P)) = v[q];
         return;
     }
+    // the partners first, all in flight together, and one post-twiddle per thread (ptw_rot): loads issued between
+    // the stores below queue behind them
+    double2 zcs[E / 2];
+    const double2 w0 = (bc != BC_P) ? __ldg(&ptw[t]) : make_double2(1.0, 0.0);
+#pragma unroll
+    for (int q = 0; q < E / 2; ++q) if (E >= PP_HOIST_ZC_MIN_E) zcs[q] = smem[lay(neg_mod<N>(t + q * P))];
 #pragma unroll
     for (int q = 0; q < E / 2; ++q) {
         const int m = t + q * P;
         const double2 zm = v[q];
-        const double2 zc = smem[lay(neg_mod<N>(m))];
+        const double2 zc = (E >= PP_HOIST_ZC_MIN_E) ? zcs[q] : smem[lay(neg_mod<N>(m))];
         if (m == 0) {
             const double2 zh = v[E / 2];
             if (bc == BC_P) {
                 *out(0) = zm;
                 *out(H) = zh;
             } else {
-                const double c4 = ptw[H].x;
+                constexpr double c4 = 0.70710678118654752440;      // cos(pi/4) = Re w_{N/2}
                 if (bc == BC_N) {
                     *out(0) = zm;
                     *out(H) = dscale(c4, zh);
@@ -260,7 +266,7 @@ __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int compl
                 *out(m) = make_double2(A.x, B.x);
                 *out((N - m)) = make_double2(A.y, B.y);
             } else {
-                const double2 wm = __ldg(&ptw[m]);
+                const double2 wm = ptw_rot<E>(w0, q, ptw, m);
                 const double2 ca = cmul(wm, A), cb = cmul(wm, B);
                 if (bc == BC_N) {
                     *out(m) = make_double2(ca.x, cb.x);
@@ -276,6 +282,35 @@ __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int compl
 }
 
 
+// L2 prefetch of a later tile (plain kernels, N >= PP_Y_PREFETCH_MIN): CTAs are handed out in the order of their linear
+// block index, so the tile PP_Y_PREFETCH indices ahead is loaded by a CTA that starts about PP_Y_PREFETCH / (resident
+// CTAs) tile lifetimes from now; one prefetch per row segment brings it into L2 meanwhile, and that CTA's load phase
+// (ncu: long-scoreboard stalls with two resident CTAs per SM) waits for L2 instead of HBM.
+#ifndef PP_Y_PREFETCH
+#define PP_Y_PREFETCH 0        // tiles ahead (0: off)
+#endif
+#ifndef PP_Y_PREFETCH_MIN
+#define PP_Y_PREFETCH_MIN 1024
+#endif
+template <int N>
+__device__ __forceinline__ void y_prefetch_ahead(const double2 *w, int nxh, bool reversed) {
+    if constexpr (PP_Y_PREFETCH > 0 && N >= PP_Y_PREFETCH_MIN) {
+        using C = typename YCfg<N>::F;
+        constexpr int E = C::E, P = C::P, T = YCfg<N>::T;
+        const int c = threadIdx.x % T, t = threadIdx.x / T;
+        if (c != 0) return;
+        const long long L = (long long)blockIdx.x + (long long)gridDim.x * blockIdx.y + PP_Y_PREFETCH;
+        if (L >= (long long)gridDim.x * gridDim.y) return;
+        const int bx = (int)(L % gridDim.x), by = (int)(L / gridDim.x);
+        const int z = reversed ? (int)gridDim.y - 1 - by : by;
+        const int col = bx * T < nxh ? bx * T : nxh - 1;
+        const double2 *base = w + (size_t)z * N * nxh + col;
+#pragma unroll
+        for (int q = 0; q < E; ++q)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(base + (t + q * P) * nxh));
+    }
+}
+
 template <int N>
 __global__ void __launch_bounds__(YCfg<N>::THREADS, YCfg<N>::MINB)
 ypass_fwd_kernel(double2 *w, int nxh, int bc, int complex_cols,
@@ -283,6 +318,7 @@ ypass_fwd_kernel(double2 *w, int nxh, int bc, int complex_cols,
     extern __shared__ double2 smem[];
     // planes from the last to the first: the x pass before this one went first to last, so the planes
     // it wrote last are still (dirty) in L2 -- they are read from there and overwritten there
+    y_prefetch_ahead<N>(w, nxh, true);
     yfwd_tile<N, false>(w, nxh, bc, complex_cols, tw, ptw, blockIdx.x, gridDim.y - 1 - blockIdx.y, smem);
 }
 
@@ -331,6 +367,8 @@ __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int compl
         // All loads first, so that they are in flight together; then the arithmetic.
         // (the upper half of v is the landing place of the second row of each pair)
         double2 yh = make_double2(0.0, 0.0);
+        // one pre-twiddle per thread, fetched with the rows; the others by rotation (ptw_rot)
+        const double2 w0 = (!cplx && bc != BC_P) ? __ldg(&ptw[t]) : make_double2(1.0, 0.0);
 #pragma unroll
         for (int q = 0; q < E / 2; ++q) {
             const int m = t + q * P;                       // 0 <= m < N/2
@@ -363,13 +401,14 @@ __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int compl
                 } else {
                     const double s1 = (bc == BC_N) ? 1.0 : sgn_of(m);  // Dirichlet: Y'_m = (-1)^m S_{N-1-m}
                     const double2 a = dscale(s1, v[q]), b = dscale(s1, v[q + E / 2]);
-                    const double2 wm = __ldg(&ptw[m]);
+                    const double2 wm = ptw_rot<E>(w0, q, ptw, m);
                     v[q] = cmul(cconj(wm), make_double2(a.x + b.y, a.y - b.x));
                     if (m > 0) {                           // conj(w_{N-m}) = i w_m
                         smem[lay(N - m)] = cmul(make_double2(-wm.y, wm.x), make_double2(b.x + a.y, b.y - a.x));
                     } else {
                         const double2 h2 = dscale((bc == BC_N) ? 1.0 : sgn_of(H), yh);
-                        smem[lay(H)] = cmul(cconj(__ldg(&ptw[H])), make_double2(h2.x + h2.y, h2.y - h2.x));
+                        constexpr double c4 = 0.70710678118654752440;          // conj(w_{N/2}) = c4 (1 + i)
+                        smem[lay(H)] = make_double2(c4 * ((h2.x + h2.y) - (h2.y - h2.x)), c4 * ((h2.x + h2.y) + (h2.y - h2.x)));
                     }
                 }
             }
@@ -406,6 +445,7 @@ __global__ void __launch_bounds__(YCfg<N>::THREADS, YCfg<N>::MINB)
 ypass_inv_kernel(double2 *w, int nxh, int bc, int complex_cols,
                  const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
     extern __shared__ double2 smem[];
+    y_prefetch_ahead<N>(w, nxh, false);
     yinv_tile<N>(w, nxh, bc, complex_cols, tw, ptw, blockIdx.x, blockIdx.y, smem);
 }
 
