@@ -143,8 +143,14 @@ int pp_plan_last_kernel_ms(pp_plan *plan, float *ms_out);
  *                    segment, s the spectral shift dz^2 (lam_x/dx^2 + lam_y/dy^2)); grids so
  *                    anisotropic that this could leave the fp64 range (dz/dx beyond ~90 with
  *                    R = 64, ~17000 with R = 32) are solved by the two-sweep kernel instead.
+ *   PP_Z_CLUSTER   : nz = 256 m, 2 <= m <= 8, Neumann / Dirichlet z: the two levels of PP_Z_PARTITION in ONE
+ *                    kernel -- the m CTAs of a line form a thread-block cluster, keep their super-segment in
+ *                    registers and exchange its first and last unknown through distributed shared memory
+ *                    (8 B read + 8 B written per point instead of 24).  PP_Z_AUTO picks it where it measured
+ *                    faster (nz = 768, 1280 ... 2048 except 1024, at least 32768 lines); this value forces it
+ *                    wherever it applies; otherwise PP_ERR_UNSUPPORTED_SIZE.
  */
-enum { PP_Z_AUTO = 0, PP_Z_SWEEP = 1, PP_Z_PARTITION = 2 };
+enum { PP_Z_AUTO = 0, PP_Z_SWEEP = 1, PP_Z_PARTITION = 2, PP_Z_CLUSTER = 3 };
 int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm);
 
 /*
@@ -158,6 +164,7 @@ int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm);
  * in the PP_K_XFWD and PP_K_XINV slots and 0 for PP_K_YFWD / PP_K_YINV.
  */
 int pp_plan_set_xy_fusion(pp_plan *plan, int enable);
+int pp_plan_set_xy_pipeline(pp_plan *plan, int planes_per_slab);
 
 /*
  * Non-homogeneous Dirichlet face values, moved to the right-hand side as PAPER.md:163 prescribes for

@@ -21,11 +21,11 @@ KERNEL_NAMES = ("x_fwd", "y_fwd", "z_solve", "y_inv", "x_inv")
 
 EXPORTS = (
     "pp_plan_create", "pp_solve", "pp_solve_host", "pp_solve_host_batch", "pp_plan_destroy", "pp_plan_workspace_bytes",
-    "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_plan_set_xy_fusion", "pp_plan_launches_per_solve", "pp_size_supported", "pp_plan_set_null_space", "pp_fold_dirichlet", "pp_strerror", "pp_version",
+    "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_plan_set_xy_fusion", "pp_plan_set_xy_pipeline", "pp_plan_launches_per_solve", "pp_size_supported", "pp_plan_set_null_space", "pp_fold_dirichlet", "pp_strerror", "pp_version",
     "pp_slab_plan_create", "pp_slab_plan_destroy", "pp_slab_local_elems", "pp_slab_chunk_elems", "pp_slab_set_exchange",
     "pp_slab_forward", "pp_slab_zsolve", "pp_slab_inverse",
 )
-PP_Z_AUTO, PP_Z_SWEEP, PP_Z_PARTITION = 0, 1, 2
+PP_Z_AUTO, PP_Z_SWEEP, PP_Z_PARTITION, PP_Z_CLUSTER = 0, 1, 2, 3
 PP_NULL_ZERO_MEAN, PP_NULL_PIN_PLANE0 = 0, 1
 
 _lib = None
@@ -68,6 +68,8 @@ def lib() -> ctypes.CDLL:
     L.pp_plan_set_z_algorithm.restype = i32
     L.pp_plan_set_xy_fusion.argtypes = [vp, i32]
     L.pp_plan_set_xy_fusion.restype = i32
+    L.pp_plan_set_xy_pipeline.argtypes = [vp, i32]
+    L.pp_plan_set_xy_pipeline.restype = i32
     L.pp_plan_launches_per_solve.argtypes = [vp]
     L.pp_plan_launches_per_solve.restype = i32
     L.pp_size_supported.argtypes = [i32, i32, i32, i32]
@@ -149,6 +151,10 @@ def pp_plan_set_z_algorithm(plan, algorithm):
 
 def pp_plan_set_xy_fusion(plan, enable):
     return lib().pp_plan_set_xy_fusion(ctypes.c_void_p(plan), int(bool(enable)))
+
+
+def pp_plan_set_xy_pipeline(plan, planes_per_slab):
+    return lib().pp_plan_set_xy_pipeline(ctypes.c_void_p(plan), int(planes_per_slab))
 
 
 def pp_plan_launches_per_solve(plan):
@@ -303,7 +309,7 @@ class Plan:
 
     def set_z_algorithm(self, algorithm):
         """'auto' | 'sweep' | 'partition' (or a PP_Z_* value)."""
-        alg = {"auto": PP_Z_AUTO, "sweep": PP_Z_SWEEP, "partition": PP_Z_PARTITION}.get(algorithm, algorithm)
+        alg = {"auto": PP_Z_AUTO, "sweep": PP_Z_SWEEP, "partition": PP_Z_PARTITION, "cluster": PP_Z_CLUSTER}.get(algorithm, algorithm)
         st = pp_plan_set_z_algorithm(self.handle, alg)
         if st != PP_SUCCESS:
             raise PittPackError(st, "pp_plan_set_z_algorithm")
@@ -312,6 +318,11 @@ class Plan:
         st = pp_plan_set_xy_fusion(self.handle, enable)
         if st != PP_SUCCESS:
             raise PittPackError(st, "pp_plan_set_xy_fusion")
+
+    def set_xy_pipeline(self, planes_per_slab: int):
+        st = pp_plan_set_xy_pipeline(self.handle, planes_per_slab)
+        if st != PP_SUCCESS:
+            raise PittPackError(st, "pp_plan_set_xy_pipeline")
 
     def fold_dirichlet(self, f, faces, stream=None):
         """``faces``: {('x'|'y'|'z', 0|1): float64 CUDA tensor of face values}; f is modified in place."""

@@ -121,6 +121,9 @@ void free_plan(pp_plan *p) {
     if (p->ev_fork) cudaEventDestroy(p->ev_fork);
     if (p->ev_join) cudaEventDestroy(p->ev_join);
     if (p->side) cudaStreamDestroy(p->side);
+    for (auto &e : p->ev_pipe) if (e) cudaEventDestroy(e);
+    if (p->ev_pipe_join) cudaEventDestroy(p->ev_pipe_join);
+    if (p->pipe) cudaStreamDestroy(p->pipe);
     for (int b = 0; b < pp_plan::NSTAGE; ++b) {
         cudaFree(p->batch_stage[b]);
         if (p->ev_in[b]) cudaEventDestroy(p->ev_in[b]);
@@ -211,7 +214,7 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
     // two-level partition (segments of 32 rows; its interface kernels carry the minors over up to 33 rows between
     // renormalisations, hence the range check): interface values [2][nK][plane] + scratch [2][nK][plane], or
     // [6][nK][plane] when the chain of super-segments is cyclic (periodic z)
-    if (!rc && long_ok && zpart_shape(nz).R == 0 && zpart_range_ok(p, 33)) {
+    if (!rc && long_ok && zpart_shape(nz).R == 0 && zpart_range_ok(p, 33) && !zpart_cluster(p)) {
         const size_t nb = sizeof(double) * (bc_z == PP_BC_PERIODIC ? 8 : 4) * (size_t)(nz / ZP_HIER_ROWS) * (size_t)nx * (size_t)ny;
         if (cudaMalloc((void **)&p->hier_scratch, nb) != cudaSuccess) { p->hier_scratch = nullptr; cudaGetLastError(); rc = PP_ERR_ALLOC; }
         else p->bytes += nb;
@@ -261,8 +264,33 @@ int pp_solve(const pp_plan *plan, const double *f, double *u, void *stream) {
     int rc;
 #define PP_MARK(i) if (prof && cudaEventRecord(mp->ev[i], st) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
     const bool fused = plan->xy_fusion && fusion_supported(plan->nx, plan->ny);
+    // x/y slab pipeline: pass A of slab k on the caller's stream, pass B of slab k on the plan's second stream as soon
+    // as A(k) is done -- beside A(k+1); the caller's stream joins at the end
+    const int pipe = (plan->xy_pipeline > 0 && plan->xy_pipeline < plan->nz && !fused) ? plan->xy_pipeline : 0;
+    auto pipelined = [&](bool fwd) -> int {
+        const int nslab = (plan->nz + pipe - 1) / pipe;
+        for (int k = 0; k < nslab; ++k) {
+            const int z0 = k * pipe, nzs = (plan->nz - z0 < pipe) ? plan->nz - z0 : pipe;
+            int r = fwd ? run_x(plan, true, f, u, st, z0, nzs) : run_y_inv(plan, u, nullptr, st, z0, nzs);
+            if (r) return r;
+            if (cudaEventRecord(mp->ev_pipe[k], st) != cudaSuccess || cudaStreamWaitEvent(mp->pipe, mp->ev_pipe[k], 0) != cudaSuccess) {
+                cudaGetLastError();
+                return PP_ERR_CUDA;
+            }
+            r = fwd ? run_y_fwd(plan, u, nullptr, mp->pipe, z0, nzs) : run_x(plan, false, u, u, mp->pipe, z0, nzs);
+            if (r) return r;
+        }
+        if (cudaEventRecord(mp->ev_pipe_join, mp->pipe) != cudaSuccess || cudaStreamWaitEvent(st, mp->ev_pipe_join, 0) != cudaSuccess) {
+            cudaGetLastError();
+            return PP_ERR_CUDA;
+        }
+        return PP_SUCCESS;
+    };
     PP_MARK(0)
-    if (fused) {
+    if (pipe) {
+        if ((rc = pipelined(true))) return rc;
+        PP_MARK(1)
+    } else if (fused) {
         if ((rc = run_fused(plan, true, f, u, st))) return rc;  // a1-a6 as tasks of one kernel
         PP_MARK(1)
     } else {
@@ -273,7 +301,10 @@ int pp_solve(const pp_plan *plan, const double *f, double *u, void *stream) {
     PP_MARK(2)
     if ((rc = run_z(plan, u, st))) return rc;                   // a7-a8: diagonal + tridiagonal solve
     PP_MARK(3)
-    if (fused) {
+    if (pipe) {
+        PP_MARK(4)
+        if ((rc = pipelined(false))) return rc;
+    } else if (fused) {
         PP_MARK(4)
         if ((rc = run_fused(plan, false, u, u, st))) return rc; // a9-a10 as tasks of one kernel
     } else {
@@ -461,10 +492,28 @@ int pp_plan_set_profiling(pp_plan *plan, int enable) {
 
 int pp_plan_set_z_algorithm(pp_plan *plan, int algorithm) {
     if (!plan) return PP_ERR_NULL;
-    if (algorithm != PP_Z_AUTO && algorithm != PP_Z_SWEEP && algorithm != PP_Z_PARTITION) return PP_ERR_INVALID_ARG;
+    if (algorithm != PP_Z_AUTO && algorithm != PP_Z_SWEEP && algorithm != PP_Z_PARTITION && algorithm != PP_Z_CLUSTER) return PP_ERR_INVALID_ARG;
+    if (algorithm == PP_Z_CLUSTER && !zpart_cluster_possible(plan)) return PP_ERR_UNSUPPORTED_SIZE;
     if (algorithm == PP_Z_PARTITION && !zpart_single_level(plan) && !plan->hier_scratch)
         return PP_ERR_UNSUPPORTED_SIZE;
     plan->z_algorithm = algorithm;
+    return PP_SUCCESS;
+}
+
+int pp_plan_set_xy_pipeline(pp_plan *plan, int planes_per_slab) {
+    if (!plan) return PP_ERR_NULL;
+    if (planes_per_slab < 0) return PP_ERR_INVALID_ARG;
+    if (int rc = check_device(plan)) return rc;
+    if (planes_per_slab > 0) {
+        if ((plan->nz + planes_per_slab - 1) / planes_per_slab > pp_plan::MAX_PIPE) return PP_ERR_INVALID_ARG;
+        if (!plan->pipe) {
+            if (cudaStreamCreateWithFlags(&plan->pipe, cudaStreamNonBlocking) != cudaSuccess) { plan->pipe = nullptr; cudaGetLastError(); return PP_ERR_CUDA; }
+            for (auto &e : plan->ev_pipe)
+                if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) { e = nullptr; cudaGetLastError(); return PP_ERR_CUDA; }
+            if (cudaEventCreateWithFlags(&plan->ev_pipe_join, cudaEventDisableTiming) != cudaSuccess) { plan->ev_pipe_join = nullptr; cudaGetLastError(); return PP_ERR_CUDA; }
+        }
+    }
+    plan->xy_pipeline = planes_per_slab;
     return PP_SUCCESS;
 }
 
@@ -515,7 +564,8 @@ int pp_plan_launches_per_solve(const pp_plan *plan) {
     const bool fused = plan->xy_fusion && fusion_supported(plan->nx, plan->ny);
     int n = fused ? 2 : 4;                                        // x/y passes
     const bool want_part = plan->z_algorithm != PP_Z_SWEEP;
-    if (want_part && !zpart_single_level(plan) && plan->hier_scratch) n += 3 + (plan->singular ? 1 : 0);
+    if (want_part && zpart_cluster(plan)) n += 1 + (plan->singular ? 1 : 0);
+    else if (want_part && !zpart_single_level(plan) && plan->hier_scratch) n += 3 + (plan->singular ? 1 : 0);
     else n += 1;
     return n;
 }

@@ -17,8 +17,12 @@ int launch_x(bool fwd, const double *in, double *out, long long npairs, int bc, 
     return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
 }
 
-int run_x(const pp_plan *p, bool fwd, const double *in, double *out, cudaStream_t st) {
-    const long long npairs = (long long)p->ny * p->nz / 2;
+int run_x(const pp_plan *p, bool fwd, const double *in, double *out, cudaStream_t st, int z0, int nzs) {
+    if (nzs < 0) nzs = p->nz;
+    const size_t off = (size_t)z0 * p->nx * p->ny;
+    in += off;
+    out += off;
+    const long long npairs = (long long)p->ny * nzs / 2;
 #define CALL_X(NN) launch_x<NN>(fwd, in, out, npairs, p->bcx, p->tw_x, p->ptw_x, st)
     PP_DISPATCH_N(p->nx, CALL_X)
 #undef CALL_X

@@ -38,9 +38,11 @@ int launch_y_inv(double *w, int nxh, int nz, int bc, int complex_cols, const dou
     return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
 }
 
-int run_y_inv(const pp_plan *p, double *w, const YRows *rows, cudaStream_t st) {
+int run_y_inv(const pp_plan *p, double *w, const YRows *rows, cudaStream_t st, int z0, int nzs) {
+    if (nzs < 0) nzs = p->nz;
+    w += (size_t)z0 * p->nx * p->ny;
     const int complex_cols = (p->bcx == PP_BC_PERIODIC && p->bcy == PP_BC_PERIODIC) ? 1 : 0;
-#define CALL_Y(NN) launch_y_inv<NN>(w, p->nx / 2, p->nz, p->bcy, complex_cols, p->tw_y, p->ptw_y, rows, st)
+#define CALL_Y(NN) launch_y_inv<NN>(w, p->nx / 2, nzs, p->bcy, complex_cols, p->tw_y, p->ptw_y, rows, st)
     PP_DISPATCH_N(p->ny, CALL_Y)
 #undef CALL_Y
 }

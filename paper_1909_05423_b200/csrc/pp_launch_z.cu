@@ -15,7 +15,12 @@ static ZPartShape plan_zpart_shape(const pp_plan *p) {
     return (z.R && zpart_range_ok(p, z.R)) ? z : ZPartShape{0, 0, 0};
 }
 
-bool zpart_single_level(const pp_plan *p) { return plan_zpart_shape(p).R != 0; }
+bool zpart_cluster_possible(const pp_plan *p) { return zpart_cluster_possible(p->nz, p->bcz == PP_BC_PERIODIC) && zpart_range_ok(p, 33); }
+bool zpart_cluster(const pp_plan *p) {
+    if (p->z_algorithm == PP_Z_CLUSTER) return zpart_cluster_possible(p);
+    return zpart_cluster_ok(p->nz, (long long)p->nx * p->ny, p->bcz == PP_BC_PERIODIC) && zpart_range_ok(p, 33);
+}
+bool zpart_single_level(const pp_plan *p) { return zpart_cluster(p) || plan_zpart_shape(p).R != 0; }
 
 int run_z(const pp_plan *p, double *w, cudaStream_t st) {
     ZParams zp;
@@ -34,7 +39,32 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
 #endif
     const bool want_part = p->z_algorithm != PP_Z_SWEEP;
     const ZPartShape zs = want_part ? plan_zpart_shape(p) : ZPartShape{0, 0, 0};
-    if (zs.R) {
+    if (want_part && zpart_cluster(p)) {
+        // two levels in one pass: a cluster of nz / 256 CTAs per line, super-segment interfaces through distributed
+        // shared memory (pp_zpart.cuh, MODE 3): one HBM read + one write per unknown
+        const ZPartShape hs = {32, ZP_HIER_ROWS / 32, 32};
+        const size_t ds = zpart_smem_bytes(hs, false, true);
+        const int nK = p->nz / ZP_HIER_ROWS;
+        const ZHier h = {nK, nullptr, nullptr, 0};
+        auto kernel = zsolve_part_kernel<32, 3, false>;
+        if (int rc = set_smem(kernel, ds)) return rc;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)((plane + hs.L - 1) / hs.L), (unsigned)nK);
+        cfg.blockDim = dim3((unsigned)(hs.L * hs.S));
+        cfg.dynamicSmemBytes = ds;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 1;
+        attr[0].val.clusterDim.y = (unsigned)nK;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        if (cudaLaunchKernelEx(&cfg, kernel, w, zp, hs.S, hs.L, h) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+        // the singular (0,0) line: column 0 only, which the cluster kernel reads but never stores
+        if (p->singular)
+            zero_mode_long_kernel<<<1, 1024, 0, st>>>(w, plane, p->nz, p->scale, p->null_space == PP_NULL_PIN_PLANE0, 0);
+    } else if (zs.R) {
         // partitioned, register-resident solve: one HBM read + one write per unknown (pp_zpart.cuh)
         const bool cyc = p->bcz == PP_BC_PERIODIC;
         const size_t ds = zpart_smem_bytes(zs, cyc);

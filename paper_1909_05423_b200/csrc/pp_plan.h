@@ -41,6 +41,12 @@ struct pp_plan {
     int *fuse_sync;            // [1 + nz] ticket + per-plane completion counters
     int fused_per_sm[2];       // resident CTAs per SM of the fused forward / inverse kernel (0: not yet asked)
     double *hier_scratch;      // [4][nz / 256][nx ny]: interface values of the two-level z solve (long lines only)
+    // x/y slab pipeline (pp_plan_set_xy_pipeline): the x and y passes run slab by slab on two streams, the y pass of
+    // slab k beside the x pass of slab k+1, so that the intermediate slab is still in L2 when it is read back
+    static constexpr int MAX_PIPE = 128;
+    int xy_pipeline;           // planes per slab (0: off)
+    cudaStream_t pipe;
+    cudaEvent_t ev_pipe[MAX_PIPE], ev_pipe_join;
     cudaStream_t side;         // long singular lines only: the zero-mode line is solved beside the two-level passes
     cudaEvent_t ev_fork, ev_join;
     cudaEvent_t ev[PP_NUM_KERNELS + 1];
@@ -83,13 +89,16 @@ inline int set_smem(K kernel, size_t smem) { return smem <= 48 * 1024 ? PP_SUCCE
 
 
 // the five passes (a1-a10 of SURVEY.md 8(a)); every launcher is stream-ordered and returns a PP_* status
-int run_x(const pp_plan *p, bool fwd, const double *in, double *out, cudaStream_t st);
-int run_y_fwd(const pp_plan *p, double *w, const YRows *slab_rows, cudaStream_t st);   // slab_rows: see pp_ypass.cuh, or NULL
-int run_y_inv(const pp_plan *p, double *w, const YRows *slab_rows, cudaStream_t st);
+// z0, nzs: the planes [z0, z0 + nzs) only (nzs < 0: all of them)
+int run_x(const pp_plan *p, bool fwd, const double *in, double *out, cudaStream_t st, int z0 = 0, int nzs = -1);
+int run_y_fwd(const pp_plan *p, double *w, const YRows *slab_rows, cudaStream_t st, int z0 = 0, int nzs = -1);   // slab_rows: see pp_ypass.cuh, or NULL
+int run_y_inv(const pp_plan *p, double *w, const YRows *slab_rows, cudaStream_t st, int z0 = 0, int nzs = -1);
 int run_z(const pp_plan *p, double *w, cudaStream_t st);
 int run_fused(const pp_plan *p, bool fwd, const double *in, double *u, cudaStream_t st);
 bool fusion_supported(int nx, int ny);
 bool zpart_range_ok(const pp_plan *p, int R);
-bool zpart_single_level(const pp_plan *p);     // does the one-CTA partitioned z kernel take this plan
+bool zpart_single_level(const pp_plan *p);     // does a one-pass partitioned z kernel (one CTA or one cluster per line) take this plan
+bool zpart_cluster(const pp_plan *p);          // ... the cluster kernel (by the plan's z_algorithm: where it pays, or wherever it applies)
+bool zpart_cluster_possible(const pp_plan *p);
 
 }  // namespace pp

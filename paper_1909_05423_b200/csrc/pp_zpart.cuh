@@ -36,6 +36,8 @@
 // same kernel on two levels (ZHier, MODE 1 / 2); everything else keeps the two-sweep kernels of
 // pp_zsolve.cuh.  The singular (0,0) line is handled by zero_mode_line exactly as there.
 #pragma once
+#include <cooperative_groups.h>
+
 #include "pp_zshape.h"
 #include "pp_zsolve.cuh"
 
@@ -51,8 +53,12 @@ namespace pp {
 //   RQ [2][L]       1 / q_R of the two blocks
 //   ZC [4][S][L]    periodic z only: the interface chain's responses to its two wrap-around couplings
 //   CL [4][L]       periodic z only: b1 times the inverse of the 2x2 closure matrix
-inline size_t zpart_smem_bytes(const ZPartShape &z, bool periodic = false) {
-    return sizeof(double) * (size_t)z.L * (2 * (z.R + 1) + 2 * z.R + 10 * z.S + 2 + (periodic ? 4 * z.S + 4 : 0));
+//   cluster mode (MODE 3) only, after RQ:  SUP [3][L] couplings a0, a1, b1 of the 256-row super-segment blocks;
+//   AB [2][L] a1, b1 of the interior R-row block; EXT [2][L] x just above / below the super-segment; XG [2][8][L] first /
+//   last unknown of every isolated super-segment of the line (each CTA of the cluster stores its two into all of them
+//   through distributed shared memory); SF [4][7][L] factored chain of super-segments (D, A D, sc, sa)
+inline size_t zpart_smem_bytes(const ZPartShape &z, bool periodic = false, bool cluster = false) {
+    return sizeof(double) * (size_t)z.L * (2 * (z.R + 1) + 2 * z.R + 10 * z.S + 2 + (periodic ? 4 * z.S + 4 : 0) + (cluster ? 51 : 0));
 }
 
 // keeps the compiler from hoisting a whole unrolled loop's shared-memory loads above it (which
@@ -87,6 +93,11 @@ __device__ __forceinline__ void zp_minors(double d0, double dint, double dlast, 
 //   MODE 2  solves each super-segment again with those neighbour values moved to the right-hand
 //           side and stores the solution                                   (8 B read + 8 B write)
 // MODE 0 is the whole line in one CTA (nK = 1).
+//   MODE 3  the same two levels in ONE pass for nK <= 8: the nK CTAs of a line form a thread-block cluster
+//           (cluster dimensions (1, nK, 1)); each keeps its isolated super-segment solution in registers, publishes
+//           its first and last unknown in its shared memory, reads the other CTAs' through distributed shared
+//           memory, solves the small chain of super-segments redundantly, and adds the neighbours' contribution to
+//           the registers by a second run of the in-CTA interface chain: 8 B read + 8 B written per point.
 struct ZHier {
     int nK;                  // super-segments per line
     double *HF, *HL;         // [nK][plane]
@@ -97,6 +108,7 @@ template <int R, int MODE, bool CYC = false>
 __global__ void __launch_bounds__(PP_ZP_MAXT, (R == 32) ? PP_ZP_MINB : PP_ZP_MINB / 2)
 zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
     static_assert(!CYC || MODE == 0, "periodic z: single-level only");
+    static_assert(MODE != 3 || R == 32, "cluster mode: super-segments of 8 x 32 rows");
     static_assert(R % 2 == 0, "the spike signs below assume an even segment length");
     extern __shared__ double zsm[];
     double *Q = zsm;                                  // [2][R+1][L]
@@ -108,6 +120,13 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
     double *RQ = PA + S * L;                          // [2][L]
     double *ZC = RQ + 2 * L;                          // [4][S][L]
     double *CL = ZC + 4 * S * L;                      // [4][L]
+    // MODE 3 (never periodic), after RQ: SUP [3][L], AB [2][L], EXT [2][L], XG [16][L], SF [28][L]
+#define ZP_SUP (RQ + 2 * L)
+#define ZP_AB (RQ + 5 * L)
+#define ZP_EXT (RQ + 7 * L)
+#define ZP_XG (RQ + 9 * L)
+#define ZP_SF (RQ + 25 * L)
+    if (MODE == 3) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");   // "I run": waited for before the first remote store
     const int SL = S * L;
     // Periodic z: every segment is an interior block and the interface chain closes on itself
     // (S interfaces instead of S - 1); see the closure below.
@@ -133,7 +152,8 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
     const int jint = cyc ? 0 : 1;                             // who tabulates the interior block
     const int jfac = cyc ? ((S >= 2) ? 1 : 0) : ((S >= 3) ? 2 : 1);   // who factors the interface matrix
     double s = -1.0;
-    if (j <= jfac && !pin) s = __ldg(p.sx + (int)(e % p.nx)) + __ldg(p.sy + (int)(e / p.nx));
+    const int jsup = (MODE == 3) ? jfac + 1 : jfac;           // MODE 3: thread jfac+1 factors the chain of super-segments
+    if (j <= jsup && !pin) s = __ldg(p.sx + (int)(e % p.nx)) + __ldg(p.sy + (int)(e / p.nx));
     double ext0 = 0.0, ext1 = 0.0;                            // x just above the CTA's first row / below its last
     if (MODE == 2 && live) {
         if (j == 0 && !top_end) ext0 = h.HL[(size_t)((K > 0) ? K - 1 : h.nK - 1) * plane + e];
@@ -178,6 +198,7 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
             const double a1 = interior ? im * rqi : 0.0, b1 = interior ? -rqi : 0.0;
             const double a0 = em * rqe;
             const double atop = top_end ? a0 : a1, abot = bot_end ? a0 : a1;
+            if (MODE == 3) { ZP_AB[l] = a1; ZP_AB[L + l] = b1; }
             // A_J obeys the Moebius recurrence A_0 = a0, A_J = a1 + b1^2 A_{J-1} / (1 - a1 A_{J-1}); carried
             // as the ratio N_J / M_J it is two FMAs per step, and the reciprocals leave the dependency chain:
             //   D_J = M_J / (M_J - vF_J N_J),   (A D)_J = N_J / (M_J - vF_J N_J)
@@ -229,6 +250,46 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
                 const double rdet = b1 / fma(k11, k22, -k12 * k21);
                 CL[l] = k22 * rdet; CL[L + l] = -k12 * rdet; CL[2 * L + l] = -k21 * rdet; CL[3 * L + l] = k11 * rdet;
             }
+        }
+    }
+    if (MODE == 3 && j == jfac + 1) {
+        // Couplings of the R S-row super-segment blocks, a = q_{n-1} / q_n and b1 = -1 / q_n at n = R S (as in
+        // zsolve_hier_interface_kernel), from the R-row block's by doubling: the minors of a Toeplitz block obey
+        // q_{2n} = q_n^2 - q_{n-1}^2 and q_{2n-1} = q_{n-1} (2 q_n - b q_{n-1}), i.e. with rho = q_{n-1} / q_n, sig = 1 / q_n:
+        //   rho' = rho (2 - b rho) / (1 - rho^2),   sig' = sig^2 / (1 - rho^2)
+        // -- log2 S steps instead of R S.  End block (d_0 = b + dl): its minors are q_n + dl q_{n-1}.
+        const double bint = -2.0 + s;
+        double qm = 1.0, qc = bint;
+#pragma unroll
+        for (int i = 1; i < R; ++i) {
+            const double qn = fma(bint, qc, -qm);
+            qm = qc; qc = qn;
+        }
+        double sig = fast_rcp(qc), rho = qm * sig;
+        for (int n = R; n < R * S; n *= 2) {
+            const double r = fast_rcp(fma(-rho, rho, 1.0));
+            const double t = rho * r;
+            rho = t * fma(-bint, rho, 2.0);
+            sig = sig * sig * r;                      // underflows to 0 for strongly dominant modes: the coupling is 0 then
+        }
+        const double dl = (p.bcz == 1) ? 1.0 : -1.0;    // b_end - b
+        const double a1 = rho, b1 = -sig;
+        const double a0 = fma(rho, fma(dl, bint, 1.0), -dl) * fast_rcp(fma(dl, rho, 1.0));
+        ZP_SUP[l] = a0; ZP_SUP[L + l] = a1; ZP_SUP[2 * L + l] = b1;
+        // factored chain of super-segments (the right-hand-side independent part of zsolve_hier_interface_kernel)
+        const int nK = h.nK;
+        const double k1 = fma(b1, b1, -a1 * a1);
+        double N = a0, M = 1.0;
+        for (int J = 0; J < nK - 1; ++J) {
+            const double vF = (J + 1 == nK - 1) ? a0 : a1, wF = (J + 1 == nK - 1) ? 0.0 : b1;
+            const double r = fast_rcp(fma(-vF, N, M));
+            const double D = M * r, AD = N * r;
+            double *f = ZP_SF + J * L + l;
+            f[0] = D; f[7 * L] = AD; f[14 * L] = D * wF; f[21 * L] = -AD * wF;
+            const double Nn = fma(k1, N, a1 * M), Mn = fma(-a1, N, M);
+            const double nrm = fast_rcp(fabs(Mn) > fabs(Nn) ? Mn : Nn);      // only the ratio N / M matters
+            N = Nn * nrm;
+            M = Mn * nrm;
         }
     }
     __syncthreads();
@@ -339,6 +400,148 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
             y[i + 1] = fma(-qc[(i + 1) * L], XR, fma(qc[(R - 2 - i) * L], XL, y[i + 1]));
             if (i % 8 == 6) zp_sched_fence();
         }
+    }
+    if (MODE == 3) {
+        // the right-hand-side part of the interface elimination, run by one thread per system (j == 0): reads YF / YL =
+        // first / last row of every segment's local solution, leaves XL / XR (x just above / below each segment) there
+        const auto chain = [&]() {
+                // interface J couples the last row of segment J with the first row of segment JF(J) = J + 1
+                // (periodic: modulo S).  The next step's coefficients are fetched before the current step's FMA chain.
+                const double *f = F + l;
+                double vL = f[0], vF = f[SL], D = f[2 * SL], A = f[3 * SL], yl = YL[l], yf = YF[((S > 1) ? L : 0) + l];
+                double pa = 0.0;
+                for (int J = 0; J < NI; ++J) {
+                    const int Jn = (J + 1 < NI) ? J + 1 : J;
+                    const int JFn = (Jn + 1 < S) ? Jn + 1 : 0;
+                    const double *fn = F + Jn * L + l;
+                    const double nvL = fn[0], nvF = fn[SL], nD = fn[2 * SL], nA = fn[3 * SL];
+                    const double nyl = YL[Jn * L + l], nyf = YF[JFn * L + l];
+                    const double Ya = fma(-vL, pa, yl);
+                    const double t = fma(-vF, Ya, yf);
+                    const double pc = D * t;
+                    pa = fma(-A, t, Ya);                 // A holds (A D)_J
+                    PC[J * L + l] = pc;
+                    PA[J * L + l] = pa;
+                    vL = nvL; vF = nvF; D = nD; A = nA; yl = nyl; yf = nyf;
+                }
+                f = F + (NI - 1) * L + l;
+                double sc = f[4 * SL], sa = f[5 * SL], pc = PC[(NI - 1) * L + l], pav = PA[(NI - 1) * L + l];
+                double cn = 0.0;
+                if (!cyc) {
+                    for (int J = NI - 1; J >= 0; --J) {
+                        const int Jn = (J > 0) ? J - 1 : 0;
+                        const double *fn = F + Jn * L + l;
+                        const double nsc = fn[4 * SL], nsa = fn[5 * SL], npc = PC[Jn * L + l], npa = PA[Jn * L + l];
+                        const double cv = fma(-sc, cn, pc);
+                        const double av = fma(-sa, cn, pav);
+                        YL[J * L + l] = cv;                  // XR of segment J   = first row of segment J+1
+                        YF[(J + 1) * L + l] = av;            // XL of segment J+1 = last row of segment J
+                        cn = cv;
+                        sc = nsc; sa = nsa; pc = npc; pav = npa;
+                    }
+                } else {
+                    // open-chain solution first (kept in PC, PA), then the closure: x = x0 - (b1 a_{S-1}) z1 - (b1 c_0) z2
+                    for (int J = NI - 1; J >= 0; --J) {
+                        const int Jn = (J > 0) ? J - 1 : 0;
+                        const double *fn = F + Jn * L + l;
+                        const double nsc = fn[4 * SL], nsa = fn[5 * SL], npc = PC[Jn * L + l], npa = PA[Jn * L + l];
+                        const double cv = fma(-sc, cn, pc);
+                        PA[J * L + l] = fma(-sa, cn, pav);
+                        PC[J * L + l] = cv;
+                        cn = cv;
+                        sc = nsc; sa = nsa; pc = npc; pav = npa;
+                    }
+                    const double x0a = PA[(S - 1) * L + l], x0c = PC[l];
+                    const double ba = fma(CL[l], x0a, CL[L + l] * x0c), bg = fma(CL[2 * L + l], x0a, CL[3 * L + l] * x0c);
+                    const double *z1c = ZC + l, *z1a = z1c + SL, *z2c = z1a + SL, *z2a = z2c + SL;
+                    for (int J = 0; J < S; ++J) {
+                        const int JF = (J + 1 < S) ? J + 1 : 0;
+                        YL[J * L + l] = fma(-ba, z1c[J * L], fma(-bg, z2c[J * L], PC[J * L + l]));    // XR of segment J
+                        YF[JF * L + l] = fma(-ba, z1a[J * L], fma(-bg, z2a[J * L], PA[J * L + l]));   // XL of segment JF
+                    }
+                }
+        };
+        // x_i = y_i - v_i xl - w_i xr with the neighbour values in YF / YL; `outer`: segment 0 / S-1 also have a neighbour
+        // outside the CTA (MODE 3: the adjacent super-segments of the cluster)
+        const auto apply = [&](bool outer) {
+            const double *qc = Q + c * (R + 1) * L + l;
+            const double xlg = (j >= 1 || cyc || outer) ? YF[j * L + l] : 0.0;
+            const double xrg = (j <= S - 2 || cyc || outer) ? YL[j * L + l] : 0.0;
+            const double rq = RQ[c * L + l];
+            const double XL = (c == 0) ? 0.0 : xlg * rq;
+            const double XR = ((c == 0 && mirror) ? xlg : xrg) * rq;
+            // x_i = y_i - v_i xl - w_i xr = y_i - (-1)^i (q_{R-1-i} XL - q_i XR)
+    #pragma unroll
+            for (int i = 0; i < R; i += 2) {
+                y[i] = fma(qc[i * L], XR, fma(-qc[(R - 1 - i) * L], XL, y[i]));
+                y[i + 1] = fma(-qc[(i + 1) * L], XR, fma(qc[(R - 2 - i) * L], XL, y[i + 1]));
+                if (i % 8 == 6) zp_sched_fence();
+            }
+        };
+        // y is the solution of the isolated super-segment.  Store its first and last unknown into the shared memory of
+        // every CTA of the cluster (distributed shared memory), then solve the chain of super-segments -- the interface
+        // system of zsolve_hier_interface_kernel, at most 7 steps, factored above -- redundantly in every CTA.
+        namespace cg = cooperative_groups;
+        cg::cluster_group cluster = cg::this_cluster();
+        const int nK = h.nK;
+        asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");        // every CTA of the cluster runs
+        if (j == 0 || j == S - 1) {
+            const double first = y[0], last = mirror ? y[0] : y[R - 1];
+            for (int q = 0; q < nK; ++q) {
+                double *dst = cluster.map_shared_rank(ZP_XG, q);
+                if (j == 0) dst[K * L + l] = first;
+                if (j == S - 1) dst[(8 + K) * L + l] = last;
+            }
+        }
+        asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+        asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+        // (no remote access after this point: a CTA may leave as soon as it is done)
+        if (j == 0) {
+            constexpr int MAXK = 8;
+            const double a0 = ZP_SUP[l], a1 = ZP_SUP[L + l], b1 = ZP_SUP[2 * L + l];
+            double pa = 0.0;
+            double pc[MAXK], pv[MAXK];
+#pragma unroll
+            for (int J = 0; J < MAXK - 1; ++J) {
+                if (J < nK - 1) {
+                    const double vL = (J == 0) ? 0.0 : b1;
+                    const double vF = (J + 1 == nK - 1) ? a0 : a1;
+                    const double *f = ZP_SF + J * L + l;
+                    const double Ya = fma(-vL, pa, ZP_XG[(8 + J) * L + l]);
+                    const double t = fma(-vF, Ya, ZP_XG[(J + 1) * L + l]);
+                    pa = fma(-f[7 * L], t, Ya);
+                    pc[J] = f[0] * t; pv[J] = pa;
+                }
+            }
+            double cn = 0.0, ext0 = 0.0, ext1 = 0.0;
+#pragma unroll
+            for (int J = MAXK - 2; J >= 0; --J) {
+                if (J < nK - 1) {
+                    const double *f = ZP_SF + J * L + l;
+                    const double cv = fma(-f[14 * L], cn, pc[J]);      // first row of super-segment J + 1
+                    const double av = fma(-f[21 * L], cn, pv[J]);      // last row of super-segment J
+                    cn = cv;
+                    if (J == K) ext1 = cv;
+                    if (J == K - 1) ext0 = av;
+                }
+            }
+            // The neighbours' values go to the right-hand side: d r = -ext0 e_first - ext1 e_last, whose local solves are
+            // -ext0 v in segment 0 and -ext1 w in segment S-1 (v_0 = w_{R-1} = a1, v_{R-1} = w_0 = b1 of the interior
+            // block; an end of the line has ext = 0).  The in-CTA chain then gives the change of every interface value.
+            const double ia = ZP_AB[l], ib = ZP_AB[L + l];
+            for (int q = 0; q < S; ++q) { YF[q * L + l] = 0.0; YL[q * L + l] = 0.0; }
+            YF[l] = -ext0 * ia;
+            YL[l] = -ext0 * ib;
+            YF[(S - 1) * L + l] += -ext1 * ib;
+            YL[(S - 1) * L + l] += -ext1 * ia;
+            ZP_EXT[l] = ext0;
+            ZP_EXT[L + l] = ext1;
+            chain();
+            YF[l] = ZP_EXT[l];                               // x just above segment 0
+            YL[(S - 1) * L + l] = ZP_EXT[L + l];             // x just below segment S-1
+        }
+        __syncthreads();
+        apply(true);
     }
     if (MODE == 1) {
         // first and last unknown of the isolated super-segment (an end of the line needs only one of them)

@@ -152,3 +152,56 @@ def test_long_line_limits():
             want = 0 if nz % 256 == 0 else 2                                              # two-level: multiples of 256
             assert pp.binding.pp_plan_set_z_algorithm(h, pp.binding.PP_Z_PARTITION) == want
             pp.binding.pp_plan_destroy(h)
+
+
+# ---- cluster kernel (PP_Z_CLUSTER): both levels of the long-line partition in one pass, super-segment interfaces
+# exchanged through distributed shared memory (include/pittpack_b200.h)
+@pytest.mark.parametrize("nz", [512, 768, 1024, 1280, 1536, 1792, 2048])
+@pytest.mark.parametrize("combo", ["PPN", "NND", "DDN", "NNN", "PDD"])
+def test_cluster_matches_oracle(nz, combo):
+    """Forced on small planes: 4 x 4 lines (half of each CTA idle) or 16 x 4 (two clusters per line set)."""
+    bc = wl.parse_bc(combo)
+    shape = (nz, 4, 4) if (nz // 256) % 2 else (nz, 4, 16)
+    h = (1.0 / shape[2], 0.8 / 4, 2.0 / nz)
+    f = wl.random_normal(shape, 2000 + nz, zero_mean=all(b in (0, 1) for b in bc))
+    ref = po.solve(f, h, bc, zdtype=np.longdouble)
+    e = rel_err(gpu_solve(f, h, bc, z_algorithm="cluster"), ref)
+    assert e <= TOL, (nz, combo, e)
+
+
+@pytest.mark.parametrize("h", [(1.0 / 32, 1.0 / 16, 1.0 / 1024), (1.0 / 1024, 1.0 / 1024, 1.0 / 16)],
+                         ids=["small-shift", "large-shift"])
+def test_cluster_conditioning(h):
+    """dz << dx: pivots near -1, the chain of super-segments at its worst conditioned; dz >> dx: minors grow like
+    |b|^32, the super-segment couplings 1 / q_256 underflow to zero (no coupling: correct)."""
+    shape = (1024, 16, 32)
+    for combo in ("PPN", "DDD"):
+        bc = wl.parse_bc(combo)
+        f = wl.random_normal(shape, 79, zero_mean=all(b in (0, 1) for b in bc))
+        ref = po.solve(f, h, bc, zdtype=np.longdouble)
+        e = rel_err(gpu_solve(f, h, bc, z_algorithm="cluster"), ref)
+        assert e <= TOL, (combo, h, e)
+
+
+def test_cluster_is_the_default_where_it_pays():
+    """256 x 128 lines of 768 rows: PP_Z_AUTO takes the cluster kernel (two launches per singular solve: the kernel and
+    the zero-mode line) and matches the oracle."""
+    import torch
+    import paper_1909_05423_b200 as pp
+    shape, h, bc = (768, 128, 256), (1.0 / 256, 1.0 / 128, 1.0 / 768), wl.parse_bc("NNN")
+    f = wl.random_normal(shape, 80, zero_mean=True)
+    plan = pp.Plan(256, 128, 768, *h, bc)
+    assert plan.launches_per_solve == 4 + 2
+    u = plan.solve(torch.from_numpy(f).cuda()).cpu().numpy()
+    plan.destroy()
+    ref = po.solve(f, h, bc)
+    assert rel_err(u, ref) <= TOL
+
+
+def test_cluster_refused_where_it_does_not_apply():
+    import paper_1909_05423_b200 as pp
+    for nz, bcz in ((256, 1), (2304, 1), (1000, 2), (1024, 0)):
+        plan = pp.Plan(16, 8, nz, 1.0, 1.0, 1.0, (1, 1, bcz))
+        with pytest.raises(pp.PittPackError):
+            plan.set_z_algorithm("cluster")
+        plan.destroy()
