@@ -115,6 +115,7 @@ __global__ void fold_face_kernel(double *f, const double *__restrict__ g, int nf
 
 void free_plan(pp_plan *p) {
     if (!p) return;
+    if (p->tw_xi != p->tw_x) cudaFree(p->tw_xi);
     cudaFree(p->tw_x); cudaFree(p->tw_y); cudaFree(p->ptw_x); cudaFree(p->ptw_y);
     cudaFree(p->sx); cudaFree(p->sy); cudaFree(p->zero_scratch); cudaFree(p->host_stage); cudaFree(p->fuse_sync); cudaFree(p->hier_scratch);
     for (auto &e : p->ev) if (e) cudaEventDestroy(e);
@@ -195,6 +196,12 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
     make_twiddles(nx, fft_E(nx, PP_X_E16_MIN), tw, ptw);
     if (!rc) rc = upload(&p->tw_x, tw, p->bytes);
     if (!rc) rc = upload(&p->ptw_x, ptw, p->bytes);
+    p->tw_xi = p->tw_x;
+    if (fft_E(nx, PP_XI_E16_MIN) != fft_E(nx, PP_X_E16_MIN)) {      // the inverse x pass runs another radix schedule
+        p->tw_xi = nullptr;
+        make_twiddles(nx, fft_E(nx, PP_XI_E16_MIN), tw, ptw);
+        if (!rc) rc = upload(&p->tw_xi, tw, p->bytes);
+    }
     make_twiddles(ny, fft_E(ny, PP_Y_E16_MIN), tw, ptw);
     if (!rc) rc = upload(&p->tw_y, tw, p->bytes);
     if (!rc) rc = upload(&p->ptw_y, ptw, p->bytes);

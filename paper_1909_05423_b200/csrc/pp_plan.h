@@ -22,6 +22,7 @@ struct pp_plan {
     int singular;
     double scale;
     double2 *tw_x, *tw_y;      // per-stage FFT twiddle tables (pp_fft.cuh, tw_stage_offset)
+    double2 *tw_xi;            // ... of the inverse x pass (== tw_x unless its radix schedule differs)
     double2 *ptw_x, *ptw_y;    // exp(-i pi m / (2n)), m in [0, n]
     double *sx, *sy;           // dz^2 lam / h^2 per packed position
     double *zero_scratch;      // [nz]

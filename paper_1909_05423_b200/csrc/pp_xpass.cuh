@@ -50,9 +50,14 @@ __device__ __forceinline__ double sgn_of(int i) { return (i & 1) ? -1.0 : 1.0; }
 #define PP_X_E16_MIN 4096     // x pass: 16 elements per thread from this length on (4096: never)
 #endif
 
-template <int N>
+#ifndef PP_XI_E16_MIN
+#define PP_XI_E16_MIN 1024    // inverse x pass: 16 elements per thread from this length on (one exchange fewer: measured
+                              // +5 % at 1024 and 2048, where the forward pass loses with it)
+#endif
+
+template <int N, bool INVERSE = false>
 struct XCfg {
-    static constexpr int E = fft_E(N, PP_X_E16_MIN);
+    static constexpr int E = fft_E(N, INVERSE ? PP_XI_E16_MIN : PP_X_E16_MIN);
     using F = FftCfg<N, E>;
     static constexpr int P = F::P;
     static constexpr int T = (256 / P) > 0 ? (256 / P) : 1;   // transforms (row pairs) per CTA; <= 4 when P >= 64
@@ -185,7 +190,7 @@ template <int N, int T, bool LDCG>
 __device__ __forceinline__ void xinv_tile(const double *in, double *out, long long pair0, long long npairs, int bc,
                                           const double2 *__restrict__ tw, const double2 *__restrict__ ptw,
                                           double2 *smem) {
-    using C = typename XCfg<N>::F;
+    using C = typename XCfg<N, true>::F;
     constexpr int E = C::E, P = C::P, H = N / 2;
     const int f = threadIdx.x / P, t = threadIdx.x % P;
     const long long pair = pair0 + f;
@@ -289,13 +294,13 @@ __device__ __forceinline__ void xinv_tile(const double *in, double *out, long lo
 }
 
 template <int N>
-__global__ void __launch_bounds__(XCfg<N>::THREADS, XCfg<N>::MINB)
+__global__ void __launch_bounds__(XCfg<N, true>::THREADS, XCfg<N, true>::MINB)
 xpass_inv_kernel(const double *in, double *out, long long npairs, int bc,
                  const double2 *__restrict__ tw, const double2 *__restrict__ ptw) {
     extern __shared__ double2 smem[];
     // rows from the last to the first: the y pass before this one went plane 0 to plane nz-1, so its
     // last planes are still in L2
-    xinv_tile<N, XCfg<N>::T, false>(in, out, (long long)(gridDim.x - 1 - blockIdx.x) * XCfg<N>::T, npairs, bc, tw, ptw, smem);
+    xinv_tile<N, XCfg<N, true>::T, false>(in, out, (long long)(gridDim.x - 1 - blockIdx.x) * XCfg<N, true>::T, npairs, bc, tw, ptw, smem);
 }
 
 }  // namespace pp

@@ -287,14 +287,15 @@ __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int compl
 // CTAs) tile lifetimes from now; one prefetch per row segment brings it into L2 meanwhile, and that CTA's load phase
 // (ncu: long-scoreboard stalls with two resident CTAs per SM) waits for L2 instead of HBM.
 #ifndef PP_Y_PREFETCH
-#define PP_Y_PREFETCH 0        // tiles ahead (0: off)
+#define PP_Y_PREFETCH 296      // tiles ahead (0: off): one wave of resident CTAs (2 x 148)
 #endif
 #ifndef PP_Y_PREFETCH_MIN
-#define PP_Y_PREFETCH_MIN 1024
+#define PP_Y_PREFETCH_MIN 1024 // measured: +7 % at N = 1024 (64-byte row segments, load phase 30 % of a tile's life),
+#define PP_Y_PREFETCH_MAX 1024 // -5 % at N = 2048 (32-byte segments: the prefetches cost L1 tag cycles the pass is short of)
 #endif
 template <int N>
 __device__ __forceinline__ void y_prefetch_ahead(const double2 *w, int nxh, bool reversed) {
-    if constexpr (PP_Y_PREFETCH > 0 && N >= PP_Y_PREFETCH_MIN) {
+    if constexpr (PP_Y_PREFETCH > 0 && N >= PP_Y_PREFETCH_MIN && N <= PP_Y_PREFETCH_MAX) {
         using C = typename YCfg<N>::F;
         constexpr int E = C::E, P = C::P, T = YCfg<N>::T;
         const int c = threadIdx.x % T, t = threadIdx.x / T;
