@@ -304,6 +304,9 @@ def run_cuda(args):
     plan = pp.Plan(nx, ny, nz, *w.h, w.bc)
     if args.fusion:
         plan.set_xy_fusion(True)
+    if args.xy_pipeline:
+        plan.set_xy_pipeline(args.xy_pipeline)
+    paired = bool(args.fusion or args.xy_pipeline)          # the x and y pass of a plane are timed as one slot
     launches = plan.launches_per_solve
     f = torch.from_numpy(w.f).cuda()
     u = torch.empty_like(f)
@@ -348,6 +351,17 @@ def run_cuda(args):
     # inside the timed region): one call per step (pp_solve_host), and a pipelined batch (pp_solve_host_batch),
     # where the copy-in of step i+1 and the copy-out of step i-1 run beside the solve of step i
     e2e_steps = max(3, min(args.steps, 10))
+    if args.no_e2e:
+        sampler.stop_flag.set()
+        sampler.join()
+        if rank == 0:
+            print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "ms_per_step": ms_step, "kernel_ms": kernel_ms,
+                              "config": {"workload": describe(w)}, "note": "--no-e2e: profiling run, not a bench line"}))
+        plan.destroy()
+        if distributed:
+            dist.barrier()
+            dist.destroy_process_group()
+        return 0
     fh = torch.from_numpy(w.f).pin_memory()
     uh = torch.empty_like(fh).pin_memory()
     plan.solve_host(fh, uh)
@@ -382,21 +396,24 @@ def run_cuda(args):
         # algorithmic bytes per point of each timed slot: 16 per pass; with x+y fusion
         # the pair's 32 sit in the x slot; the two-level z solve of long lines reads twice (24)
         slot_bytes = dict.fromkeys(pp.KERNEL_NAMES, BYTES_PER_POINT_KERNEL)
-        if args.fusion:
+        if paired:
             slot_bytes.update(x_fwd=32.0, y_fwd=0.0, y_inv=0.0, x_inv=32.0)
-        if launches - (2 if args.fusion else 4) > 1:
+        xy_launches = 2 if args.fusion else (4 * -(-nz // args.xy_pipeline) if 0 < args.xy_pipeline < nz else 4)
+        if launches - xy_launches > 2:
             slot_bytes["z_solve"] = 24.0
         dom = max((k for k in kernel_ms if slot_bytes[k] > 0), key=lambda k: kernel_ms[k] / slot_bytes[k])
         achieved = slot_bytes[dom] * npts / (kernel_ms[dom] * 1e-3) / 1e9
         solve_gbs = BYTES_PER_POINT_SOLVE * npts / (ms_step * 1e-3) / 1e9
-        wkey = args.workload + (("-" + args.bc.upper()) if args.bc else "") + ("-fused" if args.fusion else "")
+        wkey = (args.workload + (("-" + args.bc.upper()) if args.bc else "") + ("-fused" if args.fusion else "")
+                + ("-pipelined" if args.xy_pipeline else ""))
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": describe(w), "parallelism": f"replicas x{world} (no collective)",
                        "l2_policy": "inputs larger than L2 (f and u are %d MiB each)" % (npts * 8 >> 20),
-                       "in_place": False, "xy_fusion": bool(args.fusion), "kernels_per_solve": launches},
+                       "in_place": False, "library": args.lib or "default build", "xy_fusion": bool(args.fusion), "xy_pipeline_planes": int(args.xy_pipeline),
+                       "kernels_per_solve": launches},
             "clocks": sampler.result(m0, m1),
             "clocks_regions": {"per_kernel_timing": sampler.result(m2, m3), "e2e": sampler.result(m4, m5)},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": npts * 8, "d2h_bytes_per_step": npts * 8,
@@ -439,6 +456,51 @@ def run_cuda(args):
     return 0
 
 
+
+def run_probe_l2(args):
+    """SM-side throughput of the five passes with HBM out of the way: S streams, each with its own plan, solve the SAME
+    slab of the workload's x-y extent in place at the same time (a deliberate race: timing only).  The slab (<= 64 MiB)
+    stays in L2; enough CTAs are in flight to fill the machine.  Compare `equivalent_ms` with the HBM-fed solve."""
+    import torch
+    import paper_1909_05423_b200 as pp
+    w = workload_by_name(args.workload, args.bc)
+    nz, ny, nx = w.shape
+    nzs = 32
+    while nzs > 2 and nx * ny * nzs * 8 > (64 << 20):
+        nzs //= 2
+    torch.cuda.set_device(0)
+    out = {"probe": "l2_resident_concurrent_solves", "workload": describe(w), "slab": f"{nx}x{ny}x{nzs}",
+           "slab_mib": nx * ny * nzs * 8 / 2 ** 20, "runs": []}
+    for nstreams in (1, 4, 8):
+        plans = [pp.Plan(nx, ny, nzs, *w.h, w.bc) for _ in range(nstreams)]
+        u = torch.randn(nzs, ny, nx, dtype=torch.float64, device="cuda")
+        streams = [torch.cuda.Stream() for _ in range(nstreams)]
+        def go(n):
+            for _ in range(n):
+                for p, st in zip(plans, streams):
+                    p.solve(u, u, stream=st)
+        go(3)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        cur = torch.cuda.current_stream()
+        e0.record(cur)
+        for st in streams:
+            st.wait_stream(cur)
+        go(args.steps)
+        for st in streams:
+            cur.wait_stream(st)
+        e1.record(cur)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        pts = nx * ny * nzs * nstreams * args.steps
+        out["runs"].append({"streams": nstreams, "gpoints_per_s": pts / ms / 1e6,
+                            "equivalent_ms": ms * w.n_points / pts})
+        for p in plans:
+            p.destroy()
+    print(json.dumps(out))
+    return 0
+
+
 def spawn_ranks(args):
     """`python bench.py --gpus N` without a launcher: start one rank per GPU ourselves (the driver's own
     multi-GPU command is the same torch.distributed.run line)."""
@@ -461,12 +523,26 @@ def main():
     ap.add_argument("--workload", default="cfg3", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "pencil", "pencil48"])
     ap.add_argument("--bc", default=None, help="boundary conditions (x, y, z) of the cfg3 grid or a pencil, e.g. NNN; default PPN")
     ap.add_argument("--fusion", action="store_true", help="plane-wise x+y fusion through L2 (opt-in, DESIGN.md)")
+    ap.add_argument("--xy-pipeline", type=int, default=0, metavar="PLANES",
+                    help="x and y passes slab by slab on two streams, PLANES planes per slab (opt-in, DESIGN.md)")
+    ap.add_argument("--lib", default=None, metavar="PATH",
+                    help="load this build of the library instead of the default one (a variant built with "
+                         "`python -m paper_1909_05423_b200.build -D... -o PATH`: tuning switches of the kernels)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer (e2e) legs: for runs under a profiler")
+    ap.add_argument("--probe-l2", action="store_true",
+                    help="instead of the benchmark: SM-side throughput probe -- several streams solve one L2-resident "
+                         "slab of the workload's x-y extent in place at the same time (DESIGN.md section 9)")
     args = ap.parse_args()
     if args.bc is not None and (len(args.bc) != 3 or any(c not in "PNDpnd" for c in args.bc)):
         raise SystemExit("--bc: three letters out of P, N, D")
+    if args.lib:
+        import paper_1909_05423_b200.binding as binding
+        binding.LIB_PATH = os.path.abspath(args.lib)
     if args.impl == "reference":
         return run_reference(args)
+    if args.probe_l2:
+        return run_probe_l2(args)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         return spawn_ranks(args)
     return run_cuda(args)

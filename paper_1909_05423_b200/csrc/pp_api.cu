@@ -570,6 +570,8 @@ int pp_plan_launches_per_solve(const pp_plan *plan) {
     if (!plan) return 0;
     const bool fused = plan->xy_fusion && fusion_supported(plan->nx, plan->ny);
     int n = fused ? 2 : 4;                                        // x/y passes
+    if (!fused && plan->xy_pipeline > 0 && plan->xy_pipeline < plan->nz)
+        n = 4 * ((plan->nz + plan->xy_pipeline - 1) / plan->xy_pipeline);       // ... slab by slab
     const bool want_part = plan->z_algorithm != PP_Z_SWEEP;
     if (want_part && zpart_cluster(plan)) n += 1 + (plan->singular ? 1 : 0);
     else if (want_part && !zpart_single_level(plan) && plan->hier_scratch) n += 3 + (plan->singular ? 1 : 0);
