@@ -24,6 +24,14 @@ constexpr int BC_P = 0, BC_N = 1, BC_D = 2;
 struct LayoutLin {
     __device__ __forceinline__ int operator()(int i) const { return pad8(i); }
 };
+// The partner exchange of the forward pass's post-processing (element m <-> N-m) goes through the same
+// scratch UNPADDED: a quarter-warp then touches eight consecutive 16-byte slots in ascending or descending order --
+// conflict-free either way -- where the padded layout puts the pad slot inside a descending run (two-way conflicts:
+// ncu counted 3.5 M per x pass at 512 x 512 x 256, 12-14 % of its shared-memory wavefronts).  Measured: forward x pass
+// +2 % at 512, +3-4 % at 1024 and 2048.
+struct LayoutHand {
+    __device__ __forceinline__ int operator()(int i) const { return i; }
+};
 
 // synchronise the P threads of one transform inside a CTA of T transforms
 template <int P, int T>
@@ -87,6 +95,7 @@ __device__ __forceinline__ void xfwd_tile(const double *in, double *out, long lo
     double *oa = out + row * N, *ob = oa + N;
     double2 *s = smem + f * C::SMEM_ELEMS;
     const LayoutLin lay;
+    const LayoutHand hand;
     const GroupSync<P, T> sync{f};
 
     // ---- pre-processing fused into the load
@@ -111,7 +120,7 @@ __device__ __forceinline__ void xfwd_tile(const double *in, double *out, long lo
     // ---- post-processing: Hermitian separation of the two rows, twiddle, store.  The partner
     // Z_{N-m} of m in (0, N/2) lives in the upper half, so only that half goes through shared memory.
 #pragma unroll
-    for (int q = E / 2; q < E; ++q) s[lay(t + q * P)] = v[q];
+    for (int q = E / 2; q < E; ++q) s[hand(t + q * P)] = v[q];
     sync();
     if (active) {
         // the partners first, all in flight together, and one post-twiddle per thread (ptw_rot): loads issued
@@ -119,12 +128,12 @@ __device__ __forceinline__ void xfwd_tile(const double *in, double *out, long lo
         double2 zcs[E / 2];
         const double2 w0 = (bc != BC_P) ? __ldg(&ptw[t]) : make_double2(1.0, 0.0);
 #pragma unroll
-        for (int q = 0; q < E / 2; ++q) if (E >= PP_HOIST_ZC_MIN_E) zcs[q] = s[lay(neg_mod<N>(t + q * P))];
+        for (int q = 0; q < E / 2; ++q) if (E >= PP_HOIST_ZC_MIN_E) zcs[q] = s[hand(neg_mod<N>(t + q * P))];
 #pragma unroll
         for (int q = 0; q < E / 2; ++q) {
             const int m = t + q * P;                       // 0 <= m < N/2
             const double2 zm = v[q];
-            const double2 zc = (E >= PP_HOIST_ZC_MIN_E) ? zcs[q] : s[lay(neg_mod<N>(m))];
+            const double2 zc = (E >= PP_HOIST_ZC_MIN_E) ? zcs[q] : s[hand(neg_mod<N>(m))];
             if (m == 0) {
                 const double2 zh = v[E / 2];               // thread 0 also holds Z_{N/2}
                 if (bc == BC_P) {
@@ -200,6 +209,7 @@ __device__ __forceinline__ void xinv_tile(const double *in, double *out, long lo
     double *oa = out + row * N, *ob = oa + N;
     double2 *s = smem + f * C::SMEM_ELEMS;
     const LayoutLin lay;
+    const LayoutLin hand;      // the inverse pass keeps the padded layout for its hand-offs (unpadded measured 3 % slower at 16 elements per thread)
     const GroupSync<P, T> sync{f};
 
     double2 v[E];
@@ -213,10 +223,10 @@ __device__ __forceinline__ void xinv_tile(const double *in, double *out, long lo
             const double2 B = xld2<LDCG>(rb + 2 * m);
             if (m == 0) {                                              // (X_0, X_{N/2}) of both rows, all real
                 v[q] = make_double2(A.x, B.x);
-                s[lay(H)] = make_double2(A.y, B.y);
+                s[hand(H)] = make_double2(A.y, B.y);
             } else {
                 v[q] = make_double2(A.x - B.y, A.y + B.x);             // Z_m = A + i B
-                s[lay(N - m)] = make_double2(A.x + B.y, B.x - A.y);    // Z_{N-m}
+                s[hand(N - m)] = make_double2(A.x + B.y, B.x - A.y);    // Z_{N-m}
             }
         }
     } else {
@@ -247,19 +257,19 @@ __device__ __forceinline__ void xinv_tile(const double *in, double *out, long lo
             const double2 w = ptw_rot<E>(w0, q, ptw, m);
             v[q] = cmul(cconj(w), make_double2(ya + ybp, yb - yap));
             if (m > 0) {
-                s[lay(N - m)] = cmul(make_double2(-w.y, w.x), make_double2(yap + yb, ybp - ya));   // i w_m (...)
+                s[hand(N - m)] = cmul(make_double2(-w.y, w.x), make_double2(yap + yb, ybp - ya));   // i w_m (...)
             } else {
                 const double sh = (bc == BC_N) ? 1.0 : sgn_of(H);
                 constexpr double c4 = 0.70710678118654752440;              // conj(w_{N/2}) = c4 (1 + i)
                 const double hr = sh * (ha + hb), hi = sh * (hb - ha);
-                s[lay(H)] = make_double2(c4 * (hr - hi), c4 * (hr + hi));
+                s[hand(H)] = make_double2(c4 * (hr - hi), c4 * (hr + hi));
             }
         }
     }
     // every load of this row pair precedes the barrier, every store follows it: in-place safe
     sync();
 #pragma unroll
-    for (int q = E / 2; q < E; ++q) v[q] = s[lay(t + q * P)];
+    for (int q = E / 2; q < E; ++q) v[q] = s[hand(t + q * P)];
     sync();
 
     fft<N, INV>(v, t, s, tw, lay, sync);
@@ -275,13 +285,13 @@ __device__ __forceinline__ void xinv_tile(const double *in, double *out, long lo
     // 2i+1 (i < N/2) -- neighbours.  The upper half goes through shared memory to the owner of i, which
     // stores both as one 16-byte element instead of two 8-byte ones at stride 2.
 #pragma unroll
-    for (int q = E / 2; q < E; ++q) s[lay(t + q * P)] = v[q];
+    for (int q = E / 2; q < E; ++q) s[hand(t + q * P)] = v[q];
     sync();
     if (active) {
 #pragma unroll
         for (int q = 0; q < E / 2; ++q) {
             const int i = t + q * P;                                   // 0 <= i < N/2
-            const double2 lo = v[q], hi = s[lay(N - 1 - i)];
+            const double2 lo = v[q], hi = s[hand(N - 1 - i)];
             if (bc == BC_N) {
                 *reinterpret_cast<double2 *>(oa + 2 * i) = make_double2(lo.x, hi.x);
                 *reinterpret_cast<double2 *>(ob + 2 * i) = make_double2(lo.y, hi.y);
