@@ -291,6 +291,8 @@ __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int compl
 #endif
 #ifndef PP_Y_PREFETCH_MIN
 #define PP_Y_PREFETCH_MIN 1024 // measured: +7 % at N = 1024 (64-byte row segments, load phase 30 % of a tile's life),
+#endif
+#ifndef PP_Y_PREFETCH_MAX
 #define PP_Y_PREFETCH_MAX 1024 // -5 % at N = 2048 (32-byte segments: the prefetches cost L1 tag cycles the pass is short of)
 #endif
 template <int N>
