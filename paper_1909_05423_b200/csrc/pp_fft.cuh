@@ -93,6 +93,12 @@ __device__ __forceinline__ double2 cmul(double2 a, double2 b) {
     return make_double2(fma(a.x, b.x, -(a.y * b.y)), fma(a.x, b.y, a.y * b.x));
 }
 __device__ __forceinline__ double2 cconj(double2 a) { return make_double2(a.x, -a.y); }
+// x or -x by the sign bit of the high word: the (-1)^m factors of the sine transform cost an integer
+// instruction instead of a multiplication on the fp64 pipe; bit-identical to x * (+-1.0)
+__device__ __forceinline__ double neg_if(double x, bool neg) {
+    return __hiloint2double(__double2hiint(x) ^ (neg ? (int)0x80000000 : 0), __double2loint(x));
+}
+__device__ __forceinline__ double2 neg_if(double2 a, bool neg) { return make_double2(neg_if(a.x, neg), neg_if(a.y, neg)); }
 
 // multiply by W_4 = exp(DIR * i pi/2):  forward -i, inverse +i
 template <int DIR>

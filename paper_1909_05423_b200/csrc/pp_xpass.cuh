@@ -163,10 +163,10 @@ __device__ __forceinline__ void xfwd_tile(const double *in, double *out, long lo
                         oa[m] = ca.x;      ob[m] = cb.x;
                         oa[N - m] = -ca.y; ob[N - m] = -cb.y;
                     } else {
-                        const double s1 = -sgn_of(m);                  // for logical m
-                        oa[N - 1 - m] = s1 * ca.x; ob[N - 1 - m] = s1 * cb.x;
-                        // logical N-m -> position m-1, sign -(-1)^(N-m) = -(-1)^m
-                        oa[m - 1] = -s1 * ca.y;    ob[m - 1] = -s1 * cb.y;
+                        const bool odd = m & 1;                        // logical m: sign -(-1)^m
+                        oa[N - 1 - m] = neg_if(ca.x, !odd); ob[N - 1 - m] = neg_if(cb.x, !odd);
+                        // logical N-m -> position m-1: -Im with sign -(-1)^(N-m) = -(-1)^m, i.e. (-1)^m Im
+                        oa[m - 1] = neg_if(ca.y, odd);      ob[m - 1] = neg_if(cb.y, odd);
                     }
                 }
             }
@@ -252,8 +252,8 @@ __device__ __forceinline__ void xinv_tile(const double *in, double *out, long lo
 #pragma unroll
         for (int q = 0; q < E / 2; ++q) {
             const int m = t + q * P;
-            const double s1 = (bc == BC_N) ? 1.0 : sgn_of(m);           // Dirichlet: Y'_m = (-1)^m S_{N-1-m}
-            const double ya = s1 * la[q], yb = s1 * lb[q], yap = s1 * lap[q], ybp = s1 * lbp[q];
+            const bool ng = (bc == BC_D) && (m & 1);                   // Dirichlet: Y'_m = (-1)^m S_{N-1-m}
+            const double ya = neg_if(la[q], ng), yb = neg_if(lb[q], ng), yap = neg_if(lap[q], ng), ybp = neg_if(lbp[q], ng);
             const double2 w = ptw_rot<E>(w0, q, ptw, m);
             v[q] = cmul(cconj(w), make_double2(ya + ybp, yb - yap));
             if (m > 0) {

@@ -272,9 +272,9 @@ __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int compl
                     *out(m) = make_double2(ca.x, cb.x);
                     *out((N - m)) = make_double2(-ca.y, -cb.y);
                 } else {
-                    const double s1 = -sgn_of(m);
-                    *out((N - 1 - m)) = make_double2(s1 * ca.x, s1 * cb.x);
-                    *out((m - 1)) = make_double2(-s1 * ca.y, -s1 * cb.y);
+                    const bool odd = m & 1;                        // logical m -> row N-1-m, sign -(-1)^m; logical N-m -> row m-1
+                    *out((N - 1 - m)) = make_double2(neg_if(ca.x, !odd), neg_if(cb.x, !odd));
+                    *out((m - 1)) = make_double2(neg_if(ca.y, odd), neg_if(cb.y, odd));
                 }
             }
         }
@@ -402,8 +402,8 @@ __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int compl
                         smem[lay(N - m)] = make_double2(lo.x + hi.y, lo.y - hi.x);
                     }
                 } else {
-                    const double s1 = (bc == BC_N) ? 1.0 : sgn_of(m);  // Dirichlet: Y'_m = (-1)^m S_{N-1-m}
-                    const double2 a = dscale(s1, v[q]), b = dscale(s1, v[q + E / 2]);
+                    const bool ng = (bc == BC_D) && (m & 1);           // Dirichlet: Y'_m = (-1)^m S_{N-1-m}
+                    const double2 a = neg_if(v[q], ng), b = neg_if(v[q + E / 2], ng);
                     const double2 wm = ptw_rot<E>(w0, q, ptw, m);
                     v[q] = cmul(cconj(wm), make_double2(a.x + b.y, a.y - b.x));
                     if (m > 0) {                           // conj(w_{N-m}) = i w_m
@@ -437,7 +437,7 @@ __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int compl
         } else {
             const int p = (i < H) ? 2 * i : 2 * (N - 1 - i) + 1;
             if (bc == BC_N) base[p * ld] = v[q];
-            else            base[(N - 1 - p) * ld] = dscale(-sgn_of(p), v[q]);
+            else            base[(N - 1 - p) * ld] = neg_if(v[q], !(p & 1));      // x_{N-1-p} = -(-1)^p x'_p
         }
     }
 }
