@@ -55,6 +55,12 @@ __host__ __device__ constexpr int first_radix(int n, int e) {
 #define PP_E16_MIN 1024       // default schedule: 16 elements per thread from this length on
 #endif
 
+__host__ __device__ constexpr int smem_stride(int elems, int p) {
+    int s = elems;
+    while ((s * 16) % 128 != (16 * p) % 128) ++s;
+    return s;
+}
+
 template <int N, int E_ = fft_E(N, PP_E16_MIN)>
 struct FftCfg {
     static_assert(fft_length_ok(N), "N = 2^k >= 4, or 3 * 2^k / 5 * 2^k with k >= 4");
@@ -64,6 +70,11 @@ struct FftCfg {
     static constexpr int RS = stage_radix(N, E);   // radix of every stage after the first
     static constexpr int R0 = first_radix(N, E);   // first radix
     static constexpr int SMEM_ELEMS = N + N / 8;   // double2 elements per transform incl. padding
+    // x pass, several transforms per CTA: distance between their scratch areas.  With P < 8 threads per transform a
+    // quarter-warp spans 8 / P transforms, each touching P consecutive 16-byte slots: the areas are spaced so that those
+    // runs tile one 128-byte bank row (stride = 16 P bytes modulo 128) instead of overlapping (ncu: half of the
+    // 48-point x pass's shared-memory wavefronts were bank conflicts)
+    static constexpr int SMEM_STRIDE = smem_stride(N + N / 8, P);
 };
 
 // Stage twiddle tables.  Every stage after the first has radix RS (16, 8 or 4) and multiplies input r of

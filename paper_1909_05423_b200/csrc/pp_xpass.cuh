@@ -73,7 +73,7 @@ struct XCfg {
     // 8 elements per thread fit 64 registers (four CTAs per SM); 12 need about 80 (three CTAs: at 64 the 3 * 2^k
     // passes spilled up to 300 bytes per thread), 16 or 20 more than that
     static constexpr int MINB = (E <= 8) ? PP_X_MINB : ((E == 12) ? 3 : 2);
-    static constexpr size_t SMEM = size_t(T) * F::SMEM_ELEMS * sizeof(double2);
+    static constexpr size_t SMEM = size_t(T) * F::SMEM_STRIDE * sizeof(double2);
 };
 
 // ------------------------------------------------------------------------------------------
@@ -93,7 +93,7 @@ __device__ __forceinline__ void xfwd_tile(const double *in, double *out, long lo
     const long long row = active ? pair * 2 : 0;
     const double *ra = in + row * N, *rb = ra + N;
     double *oa = out + row * N, *ob = oa + N;
-    double2 *s = smem + f * C::SMEM_ELEMS;
+    double2 *s = smem + f * C::SMEM_STRIDE;
     const LayoutLin lay;
     const LayoutHand hand;
     const GroupSync<P, T> sync{f};
@@ -207,7 +207,7 @@ __device__ __forceinline__ void xinv_tile(const double *in, double *out, long lo
     const long long row = active ? pair * 2 : 0;
     const double *ra = in + row * N, *rb = ra + N;
     double *oa = out + row * N, *ob = oa + N;
-    double2 *s = smem + f * C::SMEM_ELEMS;
+    double2 *s = smem + f * C::SMEM_STRIDE;
     const LayoutLin lay;
     const LayoutLin hand;      // the inverse pass keeps the padded layout for its hand-offs (unpadded measured 3 % slower at 16 elements per thread)
     const GroupSync<P, T> sync{f};
