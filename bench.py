@@ -334,6 +334,27 @@ def run_cuda(args):
     value = whole_job_gpoints(world, npts, ms_step)
     residual = sampled_residual(u, f, w.h, w.bc)        # of the last timed solve's output
 
+    # ---- launch-bound grids (configs 1 and 2): the same K solves replayed from one CUDA graph
+    graph_ms = None
+    if npts <= (1 << 22) and world == 1:
+        gs = torch.cuda.Stream()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(gs):
+            plan.solve(f, u, stream=gs)
+            gs.synchronize()
+            with torch.cuda.graph(graph, stream=gs):
+                for _ in range(args.steps):
+                    plan.solve(f, u, stream=gs)
+            graph.replay()
+            gs.synchronize()
+            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            g0.record(gs)
+            graph.replay()
+            g1.record(gs)
+            gs.synchronize()
+        graph_ms = g0.elapsed_time(g1) / args.steps
+        del graph
+
     # ---- per-kernel durations over the same number of steps (CUDA events on the launching stream)
     plan.set_profiling(True)
     sums = dict.fromkeys(pp.KERNEL_NAMES, 0.0)
@@ -429,6 +450,7 @@ def run_cuda(args):
                                "frac_of_nominal_8TBs": solve_gbs / 8000.0},
             "kernel_ms": kernel_ms,
             "kernel_gbs": {k: slot_bytes[k] * npts / (v * 1e-3) / 1e9 for k, v in kernel_ms.items() if slot_bytes[k] > 0},
+            "graph_replay_ms_per_step": graph_ms,
             "check": {"sampled_residual_rel": residual,
                       "what": "max|A u - f| / max|f| at 200000 random cells of the last timed solve's output (eq. 3)"},
         }
