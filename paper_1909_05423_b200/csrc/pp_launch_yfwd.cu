@@ -10,6 +10,22 @@ int launch_y_fwd(double *w, int nxh, int nz, int bc, int complex_cols, const dou
                  const YRows *rows, cudaStream_t st) {
     using Y = YCfg<N>;
     const dim3 grid((unsigned)((nxh + Y::T - 1) / Y::T), (unsigned)nz);
+    if constexpr (YTma<N>::ON) {
+        if (!rows && !YStaged<N>::ON) {
+            // TMA-staged tiles: descriptors of this array (they hold its address: built per launch, on the host)
+            YTmaMaps maps;
+            bool ok;
+            ok = tma_make_rows_map(&maps.all, (const double2 *)w, nxh, N, nz, 0, 1, N, Y::T, Y_TMA_BOX_ROWS);
+            if (bc != BC_P)
+                ok = ok && tma_make_rows_map(&maps.even, (const double2 *)w, nxh, N, nz, 0, 2, N / 2, Y::T, Y_TMA_BOX_ROWS) &&
+                     tma_make_rows_map(&maps.odd, (const double2 *)w, nxh, N, nz, 1, 2, N / 2, Y::T, Y_TMA_BOX_ROWS);
+            if (!ok) return PP_ERR_CUDA;
+            auto k = ypass_fwd_tma_kernel<N>;
+            if (int rc = set_smem(k, Y::SMEM)) return rc;
+            k<<<grid, Y::THREADS, Y::SMEM, st>>>((double2 *)w, nxh, bc, complex_cols, tw, ptw, maps);
+            return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
+        }
+    }
     if (!rows && YStaged<N>::ON) {
         // persistent staged kernel: one wave of resident CTAs walks over all tiles
         using S = YStaged<N>;

@@ -22,6 +22,7 @@
 #pragma once
 #include <type_traits>
 
+#include "pp_tma.cuh"
 #include "pp_xpass.cuh"
 
 namespace pp {
@@ -176,7 +177,10 @@ __device__ __forceinline__ void yinv_stage_issue(const double2 *w, int nxh, int 
 // ld.global.cg -- for the fused x+y kernel, whose input was just written by other SMs.
 // STAGED: the tile's input was copied to `stage` by yfwd_stage_issue; `after_load` runs when every thread has its
 // input in registers (the staged kernel puts a barrier and the next tile's copies there).
-template <int N, bool LDCG, bool SLAB = false, bool STAGED = false, class Hook = NoHook>
+// (STAGED: 0 no; 1 `stage` holds the permuted sequence, position i = input i (cp.async kernel); 2 `stage` holds the rows
+// as the tensor maps of the TMA kernel deliver them: periodic: row i at i; Neumann / Dirichlet: even rows 0, 2, ... at
+// 0 .. N/2-1, odd rows 1, 3, ... at N/2 .. N-1)
+template <int N, bool LDCG, bool SLAB = false, int STAGED = 0, class Hook = NoHook>
 __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int complex_cols,
                                           const double2 *__restrict__ tw, const double2 *__restrict__ ptw,
                                           int bx, int z, double2 *smem, const YRows *rows = nullptr,
@@ -200,8 +204,14 @@ __device__ __forceinline__ void yfwd_tile(double2 *w, int nxh, int bc, int compl
 #pragma unroll
     for (int q = 0; q < E; ++q) {
         const int i = t + q * P;
-        if constexpr (STAGED) {
+        if constexpr (STAGED == 1) {
             v[q] = stage[i * T + c];
+            if (bc == BC_D && i >= H) v[q] = dscale(-1.0, v[q]);
+        } else if constexpr (STAGED == 2) {
+            // v_i = row 2i (i < H), row 2(N-1-i)+1 otherwise (Neumann); row N-1-2i, -row(2i-N) (Dirichlet): every run of
+            // consecutive i is a run of consecutive staged rows, ascending or descending (conflict-free either way)
+            const int pos = (bc == BC_P) ? i : ((bc == BC_N) ? ((i < H) ? i : H + (N - 1 - i)) : ((i < H) ? H + (H - 1 - i) : i - H));
+            v[q] = stage[pos * T + c];
             if (bc == BC_D && i >= H) v[q] = dscale(-1.0, v[q]);
         } else if (bc == BC_P) {
             v[q] = yld<LDCG>(base + i * ld);
@@ -335,7 +345,7 @@ ypass_fwd_slab_kernel(double2 *w, int nxh, int bc, int complex_cols,
 }
 
 // One CTA-wide tile of the inverse y pass (see yfwd_tile).
-template <int N, bool SLAB = false, bool STAGED = false, class Hook = NoHook>
+template <int N, bool SLAB = false, int STAGED = 0, class Hook = NoHook>
 __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int complex_cols,
                                           const double2 *__restrict__ tw, const double2 *__restrict__ ptw,
                                           int bx, int z, double2 *smem, const YRows *rows = nullptr,
@@ -488,9 +498,78 @@ ypass_staged_kernel(double2 *w, int nxh, int nz, int bc, int complex_cols,
             __syncthreads();                       // every thread has read its part of the staging buffer
             if (next < total) issue(next);
         };
-        if (FWD_DIR) yfwd_tile<N, false, false, true>(w, nxh, bc, complex_cols, tw, ptw, tile % ntx, plane_of(tile), smem, nullptr, stage, after_load);
-        else         yinv_tile<N, false, true>(w, nxh, bc, complex_cols, tw, ptw, tile % ntx, plane_of(tile), smem, nullptr, stage, after_load);
+        if (FWD_DIR) yfwd_tile<N, false, false, 1>(w, nxh, bc, complex_cols, tw, ptw, tile % ntx, plane_of(tile), smem, nullptr, stage, after_load);
+        else         yinv_tile<N, false, 1>(w, nxh, bc, complex_cols, tw, ptw, tile % ntx, plane_of(tile), smem, nullptr, stage, after_load);
     }
 }
+
+
+// ---- TMA-staged tiles (north_star item 3) -------------------------------------------------------------------
+// Used where the row segments are narrow (N = 2048: T = 2, 32 bytes): a warp-wide 16-byte load then touches 16 lines,
+// and the L1 tag stage -- one line per cycle -- costs more LSU cycles than all of the transform's shared-memory traffic
+// (DESIGN.md section 6).  Here the copy engine fetches the tile instead: one thread issues N / 256 box copies
+// (cp.async.bulk.tensor.3d, 256 rows x T*16 bytes each) into the CTA's tile buffer and everybody waits on the mbarrier;
+// the threads then read their elements from shared memory (0.125 instead of 0.5 LSU cycles per element) and the SAME
+// buffer becomes the exchange scratch -- no second buffer, the two resident CTAs per SM stay.  Stores are unchanged.
+struct YTmaMaps {
+    CUtensorMap all;      // every row of a plane: periodic forward pass, every inverse pass
+    CUtensorMap even;     // rows 0, 2, 4, ...   (Neumann / Dirichlet forward pass)
+    CUtensorMap odd;      // rows 1, 3, 5, ...
+};
+constexpr int Y_TMA_BOX_ROWS = 256;
+
+struct SyncHook {
+    __device__ __forceinline__ void operator()() const { __syncthreads(); }
+};
+
+template <int N>
+__device__ __forceinline__ void y_tma_fetch(const YTmaMaps &maps, bool permuted, int bx, int z, double2 *tile, uint64_t *bar) {
+    constexpr int T = YCfg<N>::T;
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        mbar_expect_tx(bar, (unsigned)(N * T * sizeof(double2)));
+        if (!permuted) {
+#pragma unroll
+            for (int r = 0; r < N; r += Y_TMA_BOX_ROWS) tma_load_3d(tile + r * T, &maps.all, bx * T * 2, r, z, bar);
+        } else {
+#pragma unroll
+            for (int r = 0; r < N / 2; r += Y_TMA_BOX_ROWS) {
+                tma_load_3d(tile + r * T, &maps.even, bx * T * 2, r, z, bar);
+                tma_load_3d(tile + (N / 2 + r) * T, &maps.odd, bx * T * 2, r, z, bar);
+            }
+        }
+    }
+    __syncthreads();                   // the barrier is initialised before anybody waits on it
+    mbar_wait(bar, 0);
+}
+
+template <int N>
+__global__ void __launch_bounds__(YCfg<N>::THREADS, YCfg<N>::MINB)
+ypass_fwd_tma_kernel(double2 *w, int nxh, int bc, int complex_cols, const double2 *__restrict__ tw,
+                     const double2 *__restrict__ ptw, const __grid_constant__ YTmaMaps maps) {
+    extern __shared__ __align__(128) double2 smem[];
+    __shared__ __align__(8) uint64_t bar;
+    const int z = gridDim.y - 1 - blockIdx.y;
+    y_tma_fetch<N>(maps, bc != BC_P, blockIdx.x, z, smem, &bar);
+    yfwd_tile<N, false, false, 2, SyncHook>(w, nxh, bc, complex_cols, tw, ptw, blockIdx.x, z, smem, nullptr, smem, SyncHook());
+}
+
+template <int N>
+__global__ void __launch_bounds__(YCfg<N>::THREADS, YCfg<N>::MINB)
+ypass_inv_tma_kernel(double2 *w, int nxh, int bc, int complex_cols, const double2 *__restrict__ tw,
+                     const double2 *__restrict__ ptw, const __grid_constant__ YTmaMaps maps) {
+    extern __shared__ __align__(128) double2 smem[];
+    __shared__ __align__(8) uint64_t bar;
+    y_tma_fetch<N>(maps, false, blockIdx.x, blockIdx.y, smem, &bar);
+    yinv_tile<N, false, 1, SyncHook>(w, nxh, bc, complex_cols, tw, ptw, blockIdx.x, blockIdx.y, smem, nullptr, smem, SyncHook());
+}
+
+#ifndef PP_Y_TMA_MIN
+#define PP_Y_TMA_MIN 2048         // y pass: TMA-staged tiles from this length on (powers of two only)
+#endif
+template <int N>
+struct YTma {
+    static constexpr bool ON = (N >= PP_Y_TMA_MIN) && ((N & (N - 1)) == 0) && (N % (2 * Y_TMA_BOX_ROWS) == 0);
+};
 
 }  // namespace pp
