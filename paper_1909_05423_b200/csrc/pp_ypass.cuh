@@ -565,7 +565,8 @@ ypass_inv_tma_kernel(double2 *w, int nxh, int bc, int complex_cols, const double
 }
 
 #ifndef PP_Y_TMA_MIN
-#define PP_Y_TMA_MIN 2048         // y pass: TMA-staged tiles from this length on (powers of two only)
+#define PP_Y_TMA_MIN 1024         // y pass: TMA-staged tiles from this length on (powers of two only; measured: +1-7 % at 1024,
+                                  // +7-13 % at 2048, -5 % at 512 where 128-byte row segments make the plain loads cheap)
 #endif
 template <int N>
 struct YTma {
