@@ -77,4 +77,17 @@ __device__ __forceinline__ void tma_load_3d(void *smem_dst, const CUtensorMap *m
                  : "memory");
 }
 
+// shared memory -> box at the same coordinates (bulk async group of the issuing thread)
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap *map, int x, int row, int plane, const void *smem_src) {
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(map), "r"(x), "r"(row), "r"(plane),
+                 "r"((unsigned)__cvta_generic_to_shared(smem_src))
+                 : "memory");
+}
+__device__ __forceinline__ void tma_store_commit_and_wait_read() {
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+// generic-proxy writes to shared memory made visible to the copy engine (every writing thread, before the barrier)
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 }  // namespace pp

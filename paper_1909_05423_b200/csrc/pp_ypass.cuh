@@ -345,7 +345,9 @@ ypass_fwd_slab_kernel(double2 *w, int nxh, int bc, int complex_cols,
 }
 
 // One CTA-wide tile of the inverse y pass (see yfwd_tile).
-template <int N, bool SLAB = false, int STAGED = 0, class Hook = NoHook>
+// TSTORE: the result is left in `smem` for a TMA store instead of being stored (rows in the order of the tensor maps:
+// periodic: row i at i; Neumann / Dirichlet: even rows at 0 .. N/2-1, odd rows at N/2 .. N-1, see y_tma_flush)
+template <int N, bool SLAB = false, int STAGED = 0, class Hook = NoHook, bool TSTORE = false>
 __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int complex_cols,
                                           const double2 *__restrict__ tw, const double2 *__restrict__ ptw,
                                           int bx, int z, double2 *smem, const YRows *rows = nullptr,
@@ -438,6 +440,17 @@ __device__ __forceinline__ void yinv_tile(double2 *w, int nxh, int bc, int compl
 
     fft<N, INV>(v, t, smem, tw, lay, sync);
 
+    if constexpr (TSTORE) {
+        // every exchange of the transform ended with a barrier: the tile buffer is free.  The un-permutation
+        // is the permutation of the forward pass's loads: same positions.
+#pragma unroll
+        for (int q = 0; q < E; ++q) {
+            const int i = t + q * P;
+            const int pos = (bc == BC_P) ? i : ((bc == BC_N) ? ((i < H) ? i : H + (N - 1 - i)) : ((i < H) ? H + (H - 1 - i) : i - H));
+            smem[pos * T + c] = (bc == BC_D) ? neg_if(v[q], i < H) : v[q];      // Dirichlet: x_{N-1-p} = -(-1)^p x'_p, p even for i < H
+        }
+        return;
+    }
     if (!active) return;
 #pragma unroll
     for (int q = 0; q < E; ++q) {
@@ -554,6 +567,32 @@ ypass_fwd_tma_kernel(double2 *w, int nxh, int bc, int complex_cols, const double
     yfwd_tile<N, false, false, 2, SyncHook>(w, nxh, bc, complex_cols, tw, ptw, blockIdx.x, z, smem, nullptr, smem, SyncHook());
 }
 
+// the tile buffer -> global memory by the copy engine (rows as y_tma_fetch lays them out); the CTA leaves when the
+// engine has read the buffer
+template <int N>
+__device__ __forceinline__ void y_tma_flush(const YTmaMaps &maps, bool permuted, int bx, int z, const double2 *tile) {
+    constexpr int T = YCfg<N>::T;
+    fence_proxy_async_smem();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        if (!permuted) {
+#pragma unroll
+            for (int r = 0; r < N; r += Y_TMA_BOX_ROWS) tma_store_3d(&maps.all, bx * T * 2, r, z, tile + r * T);
+        } else {
+#pragma unroll
+            for (int r = 0; r < N / 2; r += Y_TMA_BOX_ROWS) {
+                tma_store_3d(&maps.even, bx * T * 2, r, z, tile + r * T);
+                tma_store_3d(&maps.odd, bx * T * 2, r, z, tile + (N / 2 + r) * T);
+            }
+        }
+        tma_store_commit_and_wait_read();
+    }
+}
+
+#ifndef PP_Y_TMA_STORE
+#define PP_Y_TMA_STORE 0          // 1: the inverse pass's result leaves through the copy engine too.  Measured: no gain at
+#endif                            // N = 2048 (3.94 against 3.91 TB/s), -7 % at 1024: the CTA then ends with a wait for the engine
+
 template <int N>
 __global__ void __launch_bounds__(YCfg<N>::THREADS, YCfg<N>::MINB)
 ypass_inv_tma_kernel(double2 *w, int nxh, int bc, int complex_cols, const double2 *__restrict__ tw,
@@ -561,7 +600,8 @@ ypass_inv_tma_kernel(double2 *w, int nxh, int bc, int complex_cols, const double
     extern __shared__ __align__(128) double2 smem[];
     __shared__ __align__(8) uint64_t bar;
     y_tma_fetch<N>(maps, false, blockIdx.x, blockIdx.y, smem, &bar);
-    yinv_tile<N, false, 1, SyncHook>(w, nxh, bc, complex_cols, tw, ptw, blockIdx.x, blockIdx.y, smem, nullptr, smem, SyncHook());
+    yinv_tile<N, false, 1, SyncHook, PP_Y_TMA_STORE != 0>(w, nxh, bc, complex_cols, tw, ptw, blockIdx.x, blockIdx.y, smem, nullptr, smem, SyncHook());
+    if (PP_Y_TMA_STORE) y_tma_flush<N>(maps, bc != BC_P, blockIdx.x, blockIdx.y, smem);
 }
 
 #ifndef PP_Y_TMA_MIN
