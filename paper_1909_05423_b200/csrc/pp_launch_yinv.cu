@@ -19,11 +19,12 @@ int launch_y_inv(double *w, int nxh, int nz, int bc, int complex_cols, const dou
             if (bc != BC_P && PP_Y_TMA_STORE)   // the un-permuted result leaves through the even / odd row views
                 ok = ok && tma_make_rows_map(&maps.even, (const double2 *)w, nxh, N, nz, 0, 2, N / 2, Y::T, Y_TMA_BOX_ROWS) &&
                      tma_make_rows_map(&maps.odd, (const double2 *)w, nxh, N, nz, 1, 2, N / 2, Y::T, Y_TMA_BOX_ROWS);
-            if (!ok) return PP_ERR_CUDA;
-            auto k = ypass_inv_tma_kernel<N>;
-            if (int rc = set_smem(k, Y::SMEM)) return rc;
-            k<<<grid, Y::THREADS, Y::SMEM, st>>>((double2 *)w, nxh, bc, complex_cols, tw, ptw, maps);
-            return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
+            if (ok) {                       // (a driver without tensor maps: the plain kernel below)
+                auto k = ypass_inv_tma_kernel<N>;
+                if (int rc = set_smem(k, Y::SMEM)) return rc;
+                k<<<grid, Y::THREADS, Y::SMEM, st>>>((double2 *)w, nxh, bc, complex_cols, tw, ptw, maps);
+                return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
+            }
         }
     }
     if (!rows && YStaged<N>::ON) {
