@@ -15,10 +15,10 @@ int launch_y_inv(double *w, int nxh, int nz, int bc, int complex_cols, const dou
             // TMA-staged tiles: descriptors of this array (they hold its address: built per launch, on the host)
             YTmaMaps maps;
             bool ok;
-            ok = tma_make_rows_map(&maps.all, (const double2 *)w, nxh, N, nz, 0, 1, N, Y::T, Y_TMA_BOX_ROWS);
+            ok = tma_make_rows_map(&maps.all, (const double2 *)w, nxh, N, nz, 0, 1, N, Y::T, y_tma_box_rows(N));
             if (bc != BC_P && PP_Y_TMA_STORE)   // the un-permuted result leaves through the even / odd row views
-                ok = ok && tma_make_rows_map(&maps.even, (const double2 *)w, nxh, N, nz, 0, 2, N / 2, Y::T, Y_TMA_BOX_ROWS) &&
-                     tma_make_rows_map(&maps.odd, (const double2 *)w, nxh, N, nz, 1, 2, N / 2, Y::T, Y_TMA_BOX_ROWS);
+                ok = ok && tma_make_rows_map(&maps.even, (const double2 *)w, nxh, N, nz, 0, 2, N / 2, Y::T, y_tma_box_rows(N)) &&
+                     tma_make_rows_map(&maps.odd, (const double2 *)w, nxh, N, nz, 1, 2, N / 2, Y::T, y_tma_box_rows(N));
             if (ok) {                       // (a driver without tensor maps: the plain kernel below)
                 auto k = ypass_inv_tma_kernel<N>;
                 if (int rc = set_smem(k, Y::SMEM)) return rc;

@@ -529,7 +529,8 @@ struct YTmaMaps {
     CUtensorMap even;     // rows 0, 2, 4, ...   (Neumann / Dirichlet forward pass)
     CUtensorMap odd;      // rows 1, 3, 5, ...
 };
-constexpr int Y_TMA_BOX_ROWS = 256;
+// rows per box: the tensor-map limit of 256, or 128 where 256 does not divide half the column (N = 1280)
+__host__ __device__ constexpr int y_tma_box_rows(int n) { return (n / 2) % 256 == 0 ? 256 : 128; }
 
 struct SyncHook {
     __device__ __forceinline__ void operator()() const { __syncthreads(); }
@@ -537,7 +538,7 @@ struct SyncHook {
 
 template <int N>
 __device__ __forceinline__ void y_tma_fetch(const YTmaMaps &maps, bool permuted, int bx, int z, double2 *tile, uint64_t *bar) {
-    constexpr int T = YCfg<N>::T;
+    constexpr int T = YCfg<N>::T, Y_TMA_BOX_ROWS = y_tma_box_rows(N);
     if (threadIdx.x == 0) {
         mbar_init(bar, 1);
         mbar_expect_tx(bar, (unsigned)(N * T * sizeof(double2)));
@@ -571,7 +572,7 @@ ypass_fwd_tma_kernel(double2 *w, int nxh, int bc, int complex_cols, const double
 // engine has read the buffer
 template <int N>
 __device__ __forceinline__ void y_tma_flush(const YTmaMaps &maps, bool permuted, int bx, int z, const double2 *tile) {
-    constexpr int T = YCfg<N>::T;
+    constexpr int T = YCfg<N>::T, Y_TMA_BOX_ROWS = y_tma_box_rows(N);
     fence_proxy_async_smem();
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -605,12 +606,12 @@ ypass_inv_tma_kernel(double2 *w, int nxh, int bc, int complex_cols, const double
 }
 
 #ifndef PP_Y_TMA_MIN
-#define PP_Y_TMA_MIN 1024         // y pass: TMA-staged tiles from this length on (powers of two only; measured: +1-7 % at 1024,
+#define PP_Y_TMA_MIN 1024         // y pass: TMA-staged tiles from this length on (measured: +1-7 % at 1024,
                                   // +7-13 % at 2048, -5 % at 512 where 128-byte row segments make the plain loads cheap)
 #endif
 template <int N>
 struct YTma {
-    static constexpr bool ON = (N >= PP_Y_TMA_MIN) && ((N & (N - 1)) == 0) && (N % (2 * Y_TMA_BOX_ROWS) == 0);
+    static constexpr bool ON = (N >= PP_Y_TMA_MIN) && ((N / 2) % y_tma_box_rows(N) == 0);
 };
 
 }  // namespace pp
