@@ -67,6 +67,16 @@ def lap1d(n: int, bc: int) -> np.ndarray:
     return L
 
 
+def _table2(theta):
+    """Table 2: ``lam = -2 + 2 cos(theta)``, evaluated as the identical ``-4 sin^2(theta / 2)``.
+
+    The printed form cancels for small theta: at n = 2048 the lowest modes have ``1 - cos(theta) ~ 1e-6`` and
+    ``-2 + 2 cos`` in fp64 keeps only ten digits of them -- the eigenvalue the whole solve divides by (reading R27,
+    DESIGN.md; pinned against an 80-bit evaluation of the printed form in tests/test_oracle_operators.py)."""
+    sh = np.sin(0.5 * theta)
+    return -4.0 * sh * sh
+
+
 def basis(n: int, bc: int):
     """Eigenbasis of ``lap1d(n, bc)``: ``(Phi, w, lam)``.
 
@@ -88,19 +98,19 @@ def basis(n: int, bc: int):
         ang = 2.0 * np.pi * m.astype(np.float64) / n
         Phi = np.cos(ang) + 1j * np.sin(ang)
         w = np.full(n, float(n))
-        lam = -2.0 + 2.0 * np.cos(2.0 * np.pi * kk / n)
+        lam = _table2(2.0 * np.pi * np.minimum(kk, n - kk) / n)       # cos is even about pi: theta reduced to [0, pi] in integers
     elif bc == NEUMANN:
         m = ((2 * i + 1) * k) % (4 * n)
         Phi = np.cos(np.pi * m.astype(np.float64) / (2 * n))
         w = np.full(n, n / 2.0)
         w[0] = float(n)
-        lam = -2.0 + 2.0 * np.cos(np.pi * kk / n)
+        lam = _table2(np.pi * kk / n)
     elif bc == DIRICHLET:
         m = ((2 * i + 1) * (k + 1)) % (4 * n)
         Phi = np.sin(np.pi * m.astype(np.float64) / (2 * n))
         w = np.full(n, n / 2.0)
         w[n - 1] = float(n)
-        lam = -2.0 + 2.0 * np.cos(np.pi * (kk + 1.0) / n)
+        lam = _table2(np.pi * (kk + 1.0) / n)
     else:
         raise ValueError(f"unknown boundary condition {bc}")
     return Phi, w, lam

@@ -131,3 +131,19 @@ def test_second_order_convergence_on_gpu(combo):
         errs.append(float(np.sqrt(np.mean((uh - u) ** 2))))
     for coarse, fine in zip(errs[:-1], errs[1:]):
         assert abs(coarse / fine - 4.0) <= 0.3, errs
+
+
+@pytest.mark.parametrize("ny", [1024, 1280, 1536, 2048])
+@pytest.mark.parametrize("nx,combo", [(8, "PPN"), (48, "PPP"), (8, "PNN"), (16, "NPD"), (48, "PDD"), (4, "NNN")])
+def test_tma_staged_y_tiles(ny, nx, combo):
+    """The y passes of 1024 rows and more fetch their tiles through tensor maps (ypass_*_tma_kernel):
+    complex columns (x and y periodic), real pairs, every y transform type, tiles that hang over the last column
+    (nxh = 2 with four-column tiles), three planes (the forward pass walks them in reverse); out of place and in place."""
+    bc = wl.parse_bc(combo)
+    shape = (3, ny, nx)
+    h = (1.0 / nx, 1.0 / ny, 0.25)
+    f = wl.random_normal(shape, ny + nx, zero_mean=all(b in (0, 1) for b in bc))
+    w = wl.Workload(f"tma{ny}x{nx}{combo}", shape, h, bc, f)
+    u, ref = check(w)
+    u2 = gpu_solve(w.f, w.h, w.bc, in_place=True)
+    assert np.array_equal(u, u2)

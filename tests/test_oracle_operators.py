@@ -50,10 +50,44 @@ def test_lap1d_is_the_stencil(bc, n):
 def test_table2_eigenpairs(bc, n):
     Phi, w, lam = po.basis(n, bc)
     lam_paper = np.array([table2(bc, k, n) for k in range(n)])
-    np.testing.assert_allclose(lam, lam_paper, rtol=0, atol=1e-15)
+    np.testing.assert_allclose(lam, lam_paper, rtol=0, atol=4e-15)     # |lam| <= 4: a few eps of 4 (R27: -4 sin^2 against the printed -2 + 2 cos)
     for k in range(n):
         lhs = stencil_loop(Phi[:, k].copy(), bc)
         np.testing.assert_allclose(lhs, lam_paper[k] * Phi[:, k], rtol=0, atol=2e-13)
+
+
+@pytest.mark.parametrize("bc", [P, N, D])
+@pytest.mark.parametrize("n", [512, 2048, 16384])
+def test_table2_long_axes_without_cancellation(bc, n):
+    """Reading R27: the oracle evaluates Table 2's -2 + 2 cos(theta) as -4 sin^2(theta / 2).  Typed as printed but in
+    80-bit arithmetic it must agree within that evaluation's own error: |lam - printed| <= 4 eps64 |printed| + 4 eps80
+    (the 80-bit sum -2 + 2 cos carries an absolute rounding error of a few eps80 = 1.1e-19: 2e-13 relative on the lowest
+    mode of n = 2048).  The printed form in fp64 misses that by three orders (ten digits at n = 2048): the error the
+    identity removes."""
+    if np.finfo(np.longdouble).eps > 2e-19:
+        pytest.skip("no 80-bit long double on this host")
+    if n <= 2048:
+        _, _, lam = po.basis(n, bc)
+    else:                                                  # (the basis matrix of 16384^2 entries is not needed here)
+        kq = np.arange(n, dtype=np.float64)
+        lam = po._table2({P: 2.0 * np.pi * np.minimum(kq, n - kq) / n, N: np.pi * kq / n, D: np.pi * (kq + 1.0) / n}[bc])
+    k = np.arange(n, dtype=np.longdouble)
+    pi = np.longdouble("3.14159265358979323846264338327950288")
+    theta = {P: 2 * k * pi / n, N: k * pi / n, D: (k + 1) * pi / n}[bc]
+    printed = -2 + 2 * np.cos(theta)                       # PAPER.md:200-206, in long double
+    nz = np.abs(printed) > 0
+    err = np.abs(lam[nz].astype(np.longdouble) - printed[nz])
+    bound = 4 * np.finfo(np.float64).eps * np.abs(printed[nz]) + 4 * np.finfo(np.longdouble).eps
+    assert np.all(err <= bound), float((err / bound).max())
+    assert np.all(np.abs(lam[~nz]) <= 4 * np.finfo(np.longdouble).eps)
+    rel = err / np.abs(printed[nz])
+    # the printed form in fp64 loses digits on the low modes of a long axis
+    kd = np.arange(n, dtype=np.float64)
+    thd = {P: 2 * kd * np.pi / n, N: kd * np.pi / n, D: (kd + 1) * np.pi / n}[bc]
+    printed64 = -2.0 + 2.0 * np.cos(thd)
+    rel64 = np.abs((printed64[nz].astype(np.longdouble) - printed[nz]) / printed[nz])
+    if n >= 2048:
+        assert float(rel64.max()) > 1e-12 and float(rel64.max()) > 10 * float(rel.max())
 
 
 @pytest.mark.parametrize("bc", [P, N, D])
