@@ -147,3 +147,26 @@ def test_tma_staged_y_tiles(ny, nx, combo):
     u, ref = check(w)
     u2 = gpu_solve(w.f, w.h, w.bc, in_place=True)
     assert np.array_equal(u, u2)
+
+
+def test_tma_staged_under_graph_capture():
+    """The tensor maps are built on the host at launch and passed by value: a captured solve replays correctly."""
+    import torch
+    import paper_1909_05423_b200 as pp
+    shape, h, bc = (4, 1024, 16), (1.0 / 16, 1.0 / 1024, 0.25), wl.parse_bc("NDN")
+    f = wl.random_normal(shape, 5, zero_mean=False)
+    plan = pp.Plan(16, 1024, 4, *h, bc)
+    ft = torch.from_numpy(f).cuda()
+    u = torch.empty_like(ft)
+    plan.solve(ft, u)
+    torch.cuda.synchronize()
+    u.zero_()
+    g, st = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        with torch.cuda.graph(g, stream=st):
+            plan.solve(ft, u, stream=st)
+    for _ in range(2):
+        g.replay()
+    torch.cuda.synchronize()
+    assert rel_err(u.cpu().numpy(), po.solve(f, h, bc)) <= TOL
+    plan.destroy()
