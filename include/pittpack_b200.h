@@ -107,6 +107,17 @@ int pp_solve_host(pp_plan *plan, const double *f_host, double *u_host, void *str
  */
 int pp_solve_host_batch(pp_plan *plan, const double *f_host, double *u_host, int nbatch, void *stream);
 
+/*
+ * nbatch independent solves with DEVICE buffers: right-hand side i is the i-th block of nx*ny*nz doubles of f, its
+ * solution the i-th block of u (same rules as pp_solve: 16-byte aligned, u == f allowed, no partial overlap).  The
+ * transforms of all right-hand sides run as ONE launch per pass (the x and y transforms act on every xy plane
+ * independently: a batch is a taller stack of planes), the z solves one after the other:
+ * 4 + nbatch (z-solve launches) launches instead of 5 nbatch -- the use the paper itself names is a complex source,
+ * "two solves" for its real and imaginary part (reading R17), and small grids stop being launch-bound.
+ * Stream-ordered, no allocation, no synchronisation.  The x+y fusion / pipeline settings of the plan are ignored.
+ */
+int pp_solve_batch(const pp_plan *plan, const double *f, double *u, int nbatch, void *stream);
+
 /* Free the plan and everything it owns.  NULL is a no-op returning PP_SUCCESS. */
 int pp_plan_destroy(pp_plan *plan);
 

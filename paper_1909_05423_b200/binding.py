@@ -20,7 +20,7 @@ PP_NUM_KERNELS = 5
 KERNEL_NAMES = ("x_fwd", "y_fwd", "z_solve", "y_inv", "x_inv")
 
 EXPORTS = (
-    "pp_plan_create", "pp_solve", "pp_solve_host", "pp_solve_host_batch", "pp_plan_destroy", "pp_plan_workspace_bytes",
+    "pp_plan_create", "pp_solve", "pp_solve_batch", "pp_solve_host", "pp_solve_host_batch", "pp_plan_destroy", "pp_plan_workspace_bytes",
     "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_plan_set_xy_fusion", "pp_plan_set_xy_pipeline", "pp_plan_launches_per_solve", "pp_size_supported", "pp_plan_set_null_space", "pp_fold_dirichlet", "pp_strerror", "pp_version",
     "pp_slab_plan_create", "pp_slab_plan_destroy", "pp_slab_local_elems", "pp_slab_chunk_elems", "pp_slab_set_exchange",
     "pp_slab_forward", "pp_slab_zsolve", "pp_slab_inverse",
@@ -52,6 +52,8 @@ def lib() -> ctypes.CDLL:
     L.pp_plan_create.restype = i32
     L.pp_solve.argtypes = [vp, vp, vp, vp]
     L.pp_solve.restype = i32
+    L.pp_solve_batch.argtypes = [vp, vp, vp, i32, vp]
+    L.pp_solve_batch.restype = i32
     L.pp_solve_host.argtypes = [vp, vp, vp, vp]
     L.pp_solve_host.restype = i32
     L.pp_solve_host_batch.argtypes = [vp, vp, vp, i32, vp]
@@ -114,6 +116,11 @@ def pp_plan_create(nx, ny, nz, dx, dy, dz, bc_x, bc_y, bc_z):
 def pp_solve(plan, f_ptr, u_ptr, stream=0):
     return lib().pp_solve(ctypes.c_void_p(plan), ctypes.c_void_p(f_ptr), ctypes.c_void_p(u_ptr),
                           ctypes.c_void_p(stream))
+
+
+def pp_solve_batch(plan, f_ptr, u_ptr, nbatch, stream=0):
+    return lib().pp_solve_batch(ctypes.c_void_p(plan), ctypes.c_void_p(f_ptr), ctypes.c_void_p(u_ptr), int(nbatch),
+                                ctypes.c_void_p(stream))
 
 
 def pp_solve_host(plan, f_ptr, u_ptr, stream=0):
@@ -268,6 +275,24 @@ class Plan:
         st = pp_solve(self.handle, f.data_ptr(), u.data_ptr(), s.cuda_stream)
         if st != PP_SUCCESS:
             raise PittPackError(st, "pp_solve")
+        return u
+
+    def solve_batch(self, f, u=None, stream=None):
+        """f: contiguous float64 CUDA tensor (nbatch, nz, ny, nx); returns u of the same shape."""
+        import torch
+        if not (isinstance(f, torch.Tensor) and f.is_cuda and f.dtype == torch.float64 and f.is_contiguous()
+                and f.dim() == 4 and tuple(f.shape[1:]) == self.shape):
+            raise ValueError(f"f: need a contiguous float64 CUDA tensor of shape (nbatch,) + {self.shape}")
+        if u is None:
+            u = torch.empty_like(f)
+        if not (u.is_cuda and u.dtype == torch.float64 and u.is_contiguous() and u.shape == f.shape):
+            raise ValueError("u: same shape, dtype and device as f")
+        if f.device.index != self.device or u.device.index != self.device:
+            raise ValueError(f"tensors must live on cuda:{self.device}")
+        s = torch.cuda.current_stream(f.device) if stream is None else stream
+        st = pp_solve_batch(self.handle, f.data_ptr(), u.data_ptr(), f.shape[0], s.cuda_stream)
+        if st != PP_SUCCESS:
+            raise PittPackError(st, "pp_solve_batch")
         return u
 
     def solve_host(self, f_host, u_host, stream=None):

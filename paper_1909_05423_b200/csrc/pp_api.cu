@@ -215,7 +215,7 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
     if (!rc) rc = upload(&p->sy, s, p->bytes);
     p->bmax = 3.0 - smin;
     if (!rc) {
-        std::vector<double> z((size_t)nz, 0.0);
+        std::vector<double> z((size_t)nz * Z_MAX_BATCH, 0.0);
         rc = upload(&p->zero_scratch, z, p->bytes);
     }
     // two-level partition (segments of 32 rows; its interface kernels carry the minors over up to 33 rows between
@@ -323,6 +323,27 @@ int pp_solve(const pp_plan *plan, const double *f, double *u, void *stream) {
 #undef PP_MARK
     if (prof) mp->have_times = 1;
     return PP_SUCCESS;
+}
+
+int pp_solve_batch(const pp_plan *plan, const double *f, double *u, int nbatch, void *stream) {
+    if (!plan || !f || !u) return PP_ERR_NULL;
+    if (nbatch < 1) return PP_ERR_INVALID_ARG;
+    if (int rc = check_device(plan)) return rc;
+    const size_t n = (size_t)plan->nx * plan->ny * plan->nz;
+    if ((long long)plan->nz * nbatch > 0x7fffffffLL) return PP_ERR_INVALID_ARG;
+    if (((uintptr_t)f & 15) || ((uintptr_t)u & 15)) return PP_ERR_INVALID_ARG;
+    if (f != u) {
+        const uintptr_t a = (uintptr_t)f, b = (uintptr_t)u, len = n * nbatch * sizeof(double);
+        if (a < b + len && b < a + len) return PP_ERR_INVALID_ARG;     // partial overlap
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const int planes = plan->nz * nbatch;
+    int rc;
+    if ((rc = run_x(plan, true, f, u, st, 0, planes))) return rc;          // a1-a3 of every right-hand side
+    if ((rc = run_y_fwd(plan, u, nullptr, st, 0, planes))) return rc;      // a4-a6
+    if ((rc = run_z(plan, u, st, nbatch))) return rc;                      // a7-a8 (up to 64 grids per launch where one CTA holds a line)
+    if ((rc = run_y_inv(plan, u, nullptr, st, 0, planes))) return rc;      // a9
+    return run_x(plan, false, u, u, st, 0, planes);                        // a10
 }
 
 int pp_solve_host(pp_plan *plan, const double *f_host, double *u_host, void *stream) {

@@ -22,8 +22,21 @@ bool zpart_cluster(const pp_plan *p) {
 }
 bool zpart_single_level(const pp_plan *p) { return zpart_cluster(p) || plan_zpart_shape(p).R != 0; }
 
-int run_z(const pp_plan *p, double *w, cudaStream_t st) {
+static int run_z_one(const pp_plan *p, double *w, cudaStream_t st, int nbatch);
+
+int run_z(const pp_plan *p, double *w, cudaStream_t st, int nbatch) {
+    const size_t n = (size_t)p->nx * p->ny * p->nz;
+    // the one-CTA partitioned kernel takes up to Z_MAX_BATCH grids per launch (blockIdx.y); every other kernel one
+    const bool batched = p->z_algorithm != PP_Z_SWEEP && !zpart_cluster(p) && plan_zpart_shape(p).R != 0;
+    const int step = batched ? Z_MAX_BATCH : 1;
+    for (int i = 0; i < nbatch; i += step)
+        if (int rc = run_z_one(p, w + (size_t)i * n, st, (nbatch - i < step) ? nbatch - i : step)) return rc;
+    return PP_SUCCESS;
+}
+
+static int run_z_one(const pp_plan *p, double *w, cudaStream_t st, int nbatch) {
     ZParams zp;
+    zp.batch_stride = (size_t)p->nx * p->ny * p->nz;
     zp.nx = p->nx; zp.ny = p->ny; zp.nz = p->nz;
     zp.bcz = p->bcz;
     zp.singular = p->singular ? (p->null_space == PP_NULL_PIN_PLANE0 ? 2 : 1) : 0;
@@ -68,7 +81,7 @@ int run_z(const pp_plan *p, double *w, cudaStream_t st) {
         // partitioned, register-resident solve: one HBM read + one write per unknown (pp_zpart.cuh)
         const bool cyc = p->bcz == PP_BC_PERIODIC;
         const size_t ds = zpart_smem_bytes(zs, cyc);
-        const unsigned grid = (unsigned)((plane + zs.L - 1) / zs.L);
+        const dim3 grid((unsigned)((plane + zs.L - 1) / zs.L), (unsigned)nbatch);
         const ZHier none = {1, nullptr, nullptr, 0};
         auto launch = [&](auto kernel) -> int {
             if (int rc = set_smem(kernel, ds)) return rc;

@@ -25,7 +25,7 @@ struct pp_plan {
     double2 *tw_xi;            // ... of the inverse x pass (== tw_x unless its radix schedule differs)
     double2 *ptw_x, *ptw_y;    // exp(-i pi m / (2n)), m in [0, n]
     double *sx, *sy;           // dz^2 lam / h^2 per packed position
-    double *zero_scratch;      // [nz]
+    double *zero_scratch;      // [Z_MAX_BATCH][nz]
     double *host_stage;        // N doubles, created by the first pp_solve_host
     // pp_solve_host_batch: a ring of staging buffers, a copy-in and a copy-out stream, events per buffer
     static constexpr int NSTAGE = 3;
@@ -94,7 +94,7 @@ inline int set_smem(K kernel, size_t smem) { return smem <= 48 * 1024 ? PP_SUCCE
 int run_x(const pp_plan *p, bool fwd, const double *in, double *out, cudaStream_t st, int z0 = 0, int nzs = -1);
 int run_y_fwd(const pp_plan *p, double *w, const YRows *slab_rows, cudaStream_t st, int z0 = 0, int nzs = -1);   // slab_rows: see pp_ypass.cuh, or NULL
 int run_y_inv(const pp_plan *p, double *w, const YRows *slab_rows, cudaStream_t st, int z0 = 0, int nzs = -1);
-int run_z(const pp_plan *p, double *w, cudaStream_t st);
+int run_z(const pp_plan *p, double *w, cudaStream_t st, int nbatch = 1);   // nbatch grids, nx ny nz doubles apart
 int run_fused(const pp_plan *p, bool fwd, const double *in, double *u, cudaStream_t st);
 bool fusion_supported(int nx, int ny);
 bool zpart_range_ok(const pp_plan *p, int R);

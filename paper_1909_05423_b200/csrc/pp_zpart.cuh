@@ -133,6 +133,7 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
     constexpr bool cyc = CYC;
     const int NI = cyc ? S : S - 1;                   // interfaces
 
+    if (MODE == 0) w += (size_t)blockIdx.y * p.batch_stride;       // pp_solve_batch: one grid per blockIdx.y
     const int l = threadIdx.x % L, j = threadIdx.x / L;
     const size_t plane = (size_t)p.nx * p.ny;
     const size_t e = (size_t)blockIdx.x * L + l;
@@ -559,7 +560,7 @@ zsolve_part_kernel(double *w, ZParams p, int S, int L, ZHier h) {
     }
     // the warp that owns element 0 solves the singular line together (its line was never stored above)
     // (long lines: zero_mode_long_kernel does it with a whole CTA)
-    if (MODE == 0 && p.singular && blockIdx.x == 0 && threadIdx.x < 32) zero_mode_line(w, plane, p.nz, p.bcz, p.scale, p.zero_scratch, p.singular == 2);
+    if (MODE == 0 && p.singular && blockIdx.x == 0 && threadIdx.x < 32) zero_mode_line(w, plane, p.nz, p.bcz, p.scale, p.zero_scratch + (size_t)blockIdx.y * p.nz, p.singular == 2);
 }
 
 // Couples the super-segments of every line (see ZHier): one thread per mode.  The super-segment block

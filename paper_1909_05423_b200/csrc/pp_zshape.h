@@ -4,6 +4,7 @@
 
 namespace pp {
 
+constexpr int Z_MAX_BATCH = 64;   // grids per launch of the batched one-CTA partitioned kernel (pp_solve_batch)
 constexpr int Z_MAX_CK = 64;   // checkpoints per line of the two-sweep kernels (nz <= 64 Z_MAX_CK)
 
 struct ZPartShape {

@@ -36,7 +36,8 @@ struct ZParams {
     double scale;            // dz^2 / (nx ny): rhs scaling incl. the inverse-transform normalisation
     const double *sx;        // [nx]  dz^2 lam_x(kx(ix)) / dx^2
     const double *sy;        // [ny]  dz^2 lam_y(ky(j))  / dy^2
-    double *zero_scratch;    // [nz]  scratch line for the zero-mode solve
+    double *zero_scratch;    // [Z_MAX_BATCH][nz]  scratch lines for the zero-mode solve
+    size_t batch_stride;     // one-CTA partitioned kernel, pp_solve_batch: blockIdx.y selects the grid, this many doubles apart
 };
 
 

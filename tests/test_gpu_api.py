@@ -218,3 +218,32 @@ def test_host_batch_pipeline():
     assert rel_err(ub[4].numpy(), po.solve(fb[4].numpy(), w.h, w.bc)) <= TOL
     plan.solve_host_batch(fb[:2], ub[:2])              # shorter than the ring
     plan.destroy()
+
+
+@pytest.mark.parametrize("shape,combo", [((32, 32, 32), "PPD"), ((12, 48, 96), "NNN"), ((7, 16, 64), "DPN"), ((3, 1024, 8), "PNP"),
+                                         ((256, 8, 8), "NNN"), ((40, 8, 16), "PPP")])
+def test_solve_batch_is_the_solves_one_by_one(shape, combo):
+    """pp_solve_batch: the transforms of all right-hand sides in one launch per pass, the z solves one by one -- bit-identical
+    to separate pp_solve calls (singular grids: every right-hand side gets its own zero-mode fix), out of place and in place."""
+    import numpy as np
+    import torch
+    import paper_1909_05423_b200 as pp
+    from paper_1909_05423_b200 import workloads as wl
+    bc = wl.parse_bc(combo)
+    nz, ny, nx = shape
+    h = (1.0 / nx, 0.7 / ny, 1.3 / nz)
+    nb = 3
+    f = np.stack([wl.random_normal(shape, 900 + i, zero_mean=False) for i in range(nb)])
+    plan = pp.Plan(nx, ny, nz, *h, bc)
+    ft = torch.from_numpy(f).cuda()
+    one = torch.stack([plan.solve(ft[i].contiguous()) for i in range(nb)])
+    ub = plan.solve_batch(ft)
+    torch.cuda.synchronize()
+    assert torch.equal(one, ub)
+    g = ft.clone()
+    plan.solve_batch(g, g)
+    torch.cuda.synchronize()
+    assert torch.equal(one, g)
+    with pytest.raises(ValueError):
+        plan.solve_batch(ft[0])
+    plan.destroy()
