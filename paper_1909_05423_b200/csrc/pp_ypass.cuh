@@ -2,8 +2,9 @@
 //
 // On one GPU the paper's chunk exchange + data shuffle before the y transform (PAPER.md:386-403,
 // Fig. 13) becomes an in-HBM tiled transpose: a CTA owns T adjacent double2 columns (T*16 bytes
-// contiguous per row) for all ny rows of one z plane, pulls them into registers with coalesced
-// row-segment loads, runs the shared-memory FFT core down each column, and writes the tile back.
+// contiguous per row) for all ny rows of one z plane, pulls them into registers -- with coalesced
+// row-segment loads (ny <= 512), or through TMA box copies into its shared-memory tile (ny >= 1024) --,
+// runs the shared-memory FFT core down each column, and writes the tile back.
 //
 // The x-pass left every row as nx/2 double2 elements.  A double2 column is either
 //   * a complex column  -- x periodic, column >= 1: (Re, Im) of one kx mode.  With y periodic it
@@ -104,7 +105,9 @@ struct YRows {
     }
 };
 
-// ---- staged tiles (persistent kernel, north_star item 3 "staged tiles") ---------------------------------------
+// ---- double-buffered staging with cp.async (persistent kernel; a build switch, off: measured slower -- the second
+// buffer costs one of the two resident CTAs; the tiles that ARE staged go through TMA into the
+// exchange buffer itself, see ypass_*_tma_kernel below) ---------------------------------------------------------
 // A resident CTA walks over tiles and copies its NEXT tile from global into a second shared-memory buffer with
 // asynchronous 16-byte copies (cp.async / LDGSTS: no registers, no scoreboard wait) while it transforms the current
 // one -- the load latency that the plain kernels expose once per tile (ncu: long-scoreboard stalls, one or two
