@@ -394,7 +394,8 @@ def run_cuda(args):
     e1.record(stream)
     barrier()
     e2e_single_ms = max_over_ranks(e0.elapsed_time(e1), "cuda") / e2e_steps
-    nbatch = int(min(6, (3 << 30) // (npts * 8)))               # at most 3 GiB of pinned input (and as much output) per rank
+    nbatch = int(min(12, (6 << 30) // (npts * 8)))              # at most 6 GiB of pinned input (and as much output) per rank: the
+                                                                 # pipeline fills and drains once per call (one step's worth of copies)
     e2e_ms, e2e_api = e2e_single_ms, "pp_solve_host (pinned host buffers, one call per step)"
     if nbatch >= 3:
         fb = fh.unsqueeze(0).repeat(nbatch, 1, 1, 1).pin_memory()
