@@ -183,7 +183,7 @@ int pp_plan_set_xy_fusion(pp_plan *plan, int enable);
  * 512 x 512) is still in L2 when it is read back.  The caller's stream joins at the end: pp_solve stays
  * stream-ordered (and capturable).  Any grid; 0 switches it off (the default); more than 128 slabs ->
  * PP_ERR_INVALID_ARG.  Results are bit-identical.  Measured at 512 x 512 x 256: HBM traffic of a pair halves, its
- * time does not change (0.376 against 0.33 ms for the two passes run one after the other): the passes are bound
+ * time does not improve (0.36 against 0.33 ms for the two passes run one after the other): the passes are bound
  * by the SMs' shared-memory pipe, not by HBM.  Timing slots as with pp_plan_set_xy_fusion.
  */
 int pp_plan_set_xy_pipeline(pp_plan *plan, int planes_per_slab);
