@@ -54,7 +54,8 @@ enum {
     PP_ERR_UNSUPPORTED_SIZE = 2, /* nx or ny not a supported transform length, nz out of range (see pp_plan_create) */
     PP_ERR_ALLOC = 3,            /* host or device allocation failed */
     PP_ERR_CUDA = 4,             /* a CUDA runtime call or kernel launch failed (no device, bad stream, ...) */
-    PP_ERR_NULL = 5              /* a required pointer argument is NULL */
+    PP_ERR_NULL = 5,             /* a required pointer argument is NULL */
+    PP_ERR_STATIC_LIMIT = 6      /* pp_zsolve_static: nz beyond PP_STATIC_MAX_NZ, the length of its built-in work line */
 };
 
 /* The five passes of one pp_solve and their order: the timing slots of pp_plan_last_kernel_ms.  By default each
@@ -274,6 +275,47 @@ int pp_slab_forward(const pp_slab_plan *plan, const double *f_slab, double *work
 int pp_slab_zsolve(const pp_slab_plan *plan, double *pencil, void *stream);
 /* y inverse (reading through inv_src) + x inverse, result in u_slab (nz/world planes). */
 int pp_slab_inverse(const pp_slab_plan *plan, double *u_slab, void *stream);
+
+/*
+ * ---- The z solve without a plan and without any allocation -----------------------------------------------------
+ *
+ * For callers that cannot allocate device memory: an application that gave the whole GPU to its own memory pool at
+ * start-up and allows no cudaMalloc afterwards, a plug-in that only ever receives buffers, a time-critical loop (the
+ * runtime allocator synchronises the device), a process too close to out-of-memory to afford a plan.  Everything else
+ * in this header goes through a pp_plan, and pp_plan_create allocates.  pp_zsolve_static solves the tridiagonal
+ * systems of step a7-a8 (Algorithm 1; diagonal of Table 2) with what the caller
+ * passes in and one fixed work line of PP_STATIC_MAX_NZ doubles that is compiled into the library (32 KiB of every
+ * GPU that loads the library, held until the process exits).  It calls no cudaMalloc / cudaFree and no routine that
+ * allocates.  Same kernel and same arithmetic as a plan under PP_Z_SWEEP.
+ *
+ *   w         : DEVICE, nx*ny*nz doubles, x fastest: the right-hand sides after the forward x and y transforms;
+ *               overwritten by the solutions.  System (ix, j) is the strided line w[ix + nx*(j + ny*k)], k = 0..nz-1.
+ *   bc_z      : PP_BC_NEUMANN or PP_BC_DIRICHLET (first / last diagonal -1 + s / -3 + s).  Periodic z is not offered
+ *               here: PP_ERR_INVALID_ARG.
+ *   zero_mode : PP_ZERO_MODE_NONE, or -- when both transformed axes are periodic / Neumann and bc_z is Neumann, so
+ *               that system (0, 0) is singular -- which solution of it to return: zero volume mean
+ *               (what pp_solve returns by default) or zero value in plane 0 (PP_NULL_PIN_PLANE0).  Anything but
+ *               NONE with a Dirichlet bc_z is PP_ERR_INVALID_ARG.
+ *   scale     : every right-hand side is multiplied by this first (a plan uses dz^2 / (nx ny): Table 2's dz^2 and the
+ *               normalisation of the inverse transforms).
+ *   sx, sy    : DEVICE tables of nx and ny doubles, read only: the diagonal of system (ix, j) is -2 + sx[ix] + sy[j],
+ *               i.e. sx[ix] = dz^2 lambda_x(k(ix)) / dx^2 with lambda from Table 2 and k(ix) the wavenumber stored at
+ *               position ix (for this library's periodic x layout: k = 0, nx/2, 1, 1, 2, 2, ...), sy likewise.
+ *               All entries <= 0, and < 0 for every system except a singular (0, 0).
+ *   stream    : cudaStream_t as void*.  Asynchronous, stream-ordered, one kernel launch.
+ *
+ * Limit: nz <= PP_STATIC_MAX_NZ, else PP_ERR_STATIC_LIMIT and nothing is launched (longer lines need a plan).
+ * First call on a device: it looks up the device address of the work line (cudaGetSymbolAddress) and raises the
+ * kernel's shared-memory limit, once, with that device current.  Make that first call outside any stream capture.
+ * The work line is shared by every call in the process and keeps whatever the last call left in it.  Nothing in it
+ * has to start at zero -- the kernel writes each element before it reads it -- so calls that follow one another on a
+ * stream need no clearing; but two calls with zero_mode != NONE that overlap on the GPU (different streams, other
+ * threads, no ordering between them) write the same line and corrupt each other's (0, 0) system.  Order them.
+ */
+#define PP_STATIC_MAX_NZ 4096
+enum { PP_ZERO_MODE_NONE = 0, PP_ZERO_MODE_ZERO_MEAN = 1, PP_ZERO_MODE_PIN_PLANE0 = 2 };
+int pp_zsolve_static(double *w, int nx, int ny, int nz, int bc_z, int zero_mode, double scale,
+                     const double *sx, const double *sy, void *stream);
 
 /* Static, NUL-terminated description of a status code. */
 const char *pp_strerror(int status);

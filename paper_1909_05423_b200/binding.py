@@ -24,7 +24,11 @@ EXPORTS = (
     "pp_plan_set_profiling", "pp_plan_last_kernel_ms", "pp_plan_set_z_algorithm", "pp_plan_set_xy_fusion", "pp_plan_set_xy_pipeline", "pp_plan_launches_per_solve", "pp_size_supported", "pp_plan_set_null_space", "pp_fold_dirichlet", "pp_strerror", "pp_version",
     "pp_slab_plan_create", "pp_slab_plan_destroy", "pp_slab_local_elems", "pp_slab_chunk_elems", "pp_slab_set_exchange",
     "pp_slab_forward", "pp_slab_zsolve", "pp_slab_inverse",
+    "pp_zsolve_static",
 )
+PP_STATIC_MAX_NZ = 4096
+PP_ERR_STATIC_LIMIT = 6
+PP_ZERO_MODE_NONE, PP_ZERO_MODE_ZERO_MEAN, PP_ZERO_MODE_PIN_PLANE0 = 0, 1, 2
 PP_Z_AUTO, PP_Z_SWEEP, PP_Z_PARTITION, PP_Z_CLUSTER = 0, 1, 2, 3
 PP_NULL_ZERO_MEAN, PP_NULL_PIN_PLANE0 = 0, 1
 
@@ -96,6 +100,8 @@ def lib() -> ctypes.CDLL:
     L.pp_slab_zsolve.restype = i32
     L.pp_slab_inverse.argtypes = [vp, vp, vp]
     L.pp_slab_inverse.restype = i32
+    L.pp_zsolve_static.argtypes = [vp, i32, i32, i32, i32, i32, dbl, vp, vp, vp]
+    L.pp_zsolve_static.restype = i32
     L.pp_strerror.argtypes = [i32]
     L.pp_strerror.restype = ctypes.c_char_p
     L.pp_version.argtypes = []
@@ -220,6 +226,13 @@ def pp_slab_zsolve(plan, pencil_ptr, stream=0):
 
 def pp_slab_inverse(plan, u_ptr, stream=0):
     return lib().pp_slab_inverse(ctypes.c_void_p(plan), ctypes.c_void_p(u_ptr), ctypes.c_void_p(stream))
+
+
+def pp_zsolve_static(w_ptr, nx, ny, nz, bc_z, zero_mode, scale, sx_ptr, sy_ptr, stream=0):
+    """The plan-free z solve for callers that may not allocate device memory (see the header): w, sx, sy are
+    device addresses; nz <= PP_STATIC_MAX_NZ, else PP_ERR_STATIC_LIMIT."""
+    return lib().pp_zsolve_static(ctypes.c_void_p(w_ptr), int(nx), int(ny), int(nz), int(bc_z), int(zero_mode),
+                                  float(scale), ctypes.c_void_p(sx_ptr), ctypes.c_void_p(sy_ptr), ctypes.c_void_p(stream))
 
 
 def strerror(status: int) -> str:

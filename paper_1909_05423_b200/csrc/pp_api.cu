@@ -154,6 +154,7 @@ const char *pp_strerror(int status) {
         case PP_ERR_ALLOC: return "allocation failed";
         case PP_ERR_CUDA: return "CUDA runtime or launch error (is a CUDA device present?)";
         case PP_ERR_NULL: return "null pointer argument";
+        case PP_ERR_STATIC_LIMIT: return "nz is beyond PP_STATIC_MAX_NZ = 4096, the fixed work line of pp_zsolve_static (longer lines need a plan)";
         default: return "unknown status";
     }
 }

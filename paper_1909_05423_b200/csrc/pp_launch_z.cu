@@ -1,5 +1,8 @@
 // z-solve launcher (a7-a8): picks the partitioned, two-level or two-sweep kernels.
+#include <climits>
 #include <cmath>
+#include <cstdint>
+#include <mutex>
 
 #include "pp_plan.h"
 #include "pp_zsolve.cuh"
@@ -158,3 +161,86 @@ static int run_z_one(const pp_plan *p, double *w, cudaStream_t st, int nbatch) {
 }
 
 }  // namespace pp
+
+// ------------------------------------------------------------------------------------------------------------------
+// pp_zsolve_static (include/pittpack_b200.h): the z solve (a7-a8) for callers that must not allocate device memory.
+//
+// Who that is: code running where a cudaMalloc is off limits -- a host application that handed all of the GPU's memory
+// to its own pool at start-up and forbids the runtime allocator afterwards, a plug-in that is only ever given buffers,
+// a latency-critical loop (cudaMalloc and cudaFree synchronise the whole device), or a process that is close to
+// out of memory and cannot afford a plan.  Every other entry point of this library needs a pp_plan, and
+// pp_plan_create uploads its tables with cudaMalloc.  This one takes no plan: the caller passes the grid, the two
+// shift tables and the right-hand sides, and the only memory the kernel needs beyond those -- the work line of the
+// singular (kx, ky) = (0, 0) system (zero_mode_line, pp_zsolve.cuh) -- is the fixed array below, which is part of the
+// loaded library image: PP_STATIC_MAX_NZ doubles (32 KiB) on every GPU that loads the library, until the process exits.
+//
+// The kernel is the two-sweep Thomas kernel of the plan path (zsolve_thomas_kernel<16, 128>, the one PP_Z_SWEEP
+// selects), unchanged; only where its scratch pointer comes from differs.  It lives in this file because the kernel
+// templates of pp_zsolve.cuh can be included by one translation unit only.
+namespace {
+
+// The work line.  In HOST code this name is only a handle for the runtime (cudaGetSymbolAddress, cudaMemcpyToSymbol):
+// its host-side address is not a device address and must never be handed to a kernel.  static_setup() below asks the
+// runtime for the real address, once per device.
+static __device__ __align__(256) double g_static_zero_line[PP_STATIC_MAX_NZ];
+
+constexpr int CB = 16, TH = 128;                      // checkpoint spacing and threads per CTA, as pp_launch_z.cu
+constexpr int MAX_DEVICES = 64;
+
+constexpr size_t smem_bytes(int nz) { return (size_t)(((nz + 1) / 2 + CB - 1) / CB) * TH * sizeof(double); }
+
+std::mutex g_static_mutex;
+double *g_static_addr[MAX_DEVICES];                   // device address of g_static_zero_line per device; NULL: not set up yet
+
+// Once per device, with that device current: the address of the work line on this device, and the kernel's opt-in
+// to the dynamic shared memory of the longest line (a function attribute; no device memory is allocated).
+int static_setup(int dev, double **line) {
+    if (dev < 0 || dev >= MAX_DEVICES) return PP_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+        double *ptr = nullptr;
+        if (cudaGetSymbolAddress((void **)&ptr, g_static_zero_line) != cudaSuccess || !ptr) {
+            cudaGetLastError();
+            return PP_ERR_CUDA;
+        }
+        // through the library's registry of per-kernel limits, so that a plan using the same kernel never lowers it again
+        if (int rc = pp::set_smem_once((const void *)pp::zsolve_thomas_kernel<CB, TH>, smem_bytes(PP_STATIC_MAX_NZ))) return rc;
+        g_static_addr[dev] = ptr;
+    }
+    *line = g_static_addr[dev];
+    return PP_SUCCESS;
+}
+
+}  // namespace
+
+extern "C" int pp_zsolve_static(double *w, int nx, int ny, int nz, int bc_z, int zero_mode, double scale,
+                                const double *sx, const double *sy, void *stream) {
+    // argument checks first: none of them needs a device
+    if (!w || !sx || !sy) return PP_ERR_NULL;
+    if (nx < 1 || ny < 1 || nz < 2) return PP_ERR_INVALID_ARG;
+    if (bc_z != PP_BC_NEUMANN && bc_z != PP_BC_DIRICHLET) return PP_ERR_INVALID_ARG;      // periodic z: not served here
+    if (zero_mode != PP_ZERO_MODE_NONE && zero_mode != PP_ZERO_MODE_ZERO_MEAN && zero_mode != PP_ZERO_MODE_PIN_PLANE0)
+        return PP_ERR_INVALID_ARG;
+    if (zero_mode != PP_ZERO_MODE_NONE && bc_z != PP_BC_NEUMANN) return PP_ERR_INVALID_ARG; // a Dirichlet axis: never singular
+    if (!std::isfinite(scale)) return PP_ERR_INVALID_ARG;
+    if (nz > PP_STATIC_MAX_NZ) return PP_ERR_STATIC_LIMIT;                                  // the fixed work line is this long
+    if (((uintptr_t)w & 7) || ((uintptr_t)sx & 7) || ((uintptr_t)sy & 7)) return PP_ERR_INVALID_ARG;
+    const long long plane = (long long)nx * ny;
+    if ((plane + TH - 1) / TH > (long long)INT_MAX) return PP_ERR_INVALID_ARG;
+
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
+    double *line = nullptr;
+    if (int rc = static_setup(dev, &line)) return rc;
+
+    pp::ZParams zp;
+    zp.nx = nx; zp.ny = ny; zp.nz = nz;
+    zp.bcz = bc_z;
+    zp.singular = zero_mode;
+    zp.scale = scale;
+    zp.sx = sx; zp.sy = sy;
+    zp.zero_scratch = line;            // the device address from cudaGetSymbolAddress, not the symbol's host-side name
+    zp.batch_stride = 0;
+    pp::zsolve_thomas_kernel<CB, TH><<<(unsigned)((plane + TH - 1) / TH), TH, smem_bytes(nz), (cudaStream_t)stream>>>(w, zp);
+    return cudaGetLastError() == cudaSuccess ? PP_SUCCESS : PP_ERR_CUDA;
+}
