@@ -122,3 +122,43 @@ def test_longdouble_z_option():
     u_ld = po.solve(f, h, bc, zdtype=np.longdouble)
     assert u_ld.dtype == np.float64
     np.testing.assert_allclose(u_ld, u, rtol=0, atol=1e-12 * np.max(np.abs(u)))
+
+
+@pytest.mark.parametrize("long_axis", ["x", "y"])
+@pytest.mark.parametrize("bc_long", [P, N, D], ids=lambda b: "PND"[b])
+def test_closed_form_low_modes_on_a_long_axis(long_axis, bc_long, monkeypatch):
+    """Solve-level pin of reading R27: on a 2048-point transform axis the lowest modes have
+    lam = -2 + 2 cos(theta) ~ -1e-5, and u = f / lam divides by it.  Expected values: Table 2 AS PRINTED,
+    evaluated in 60-digit decimal arithmetic (tests/hp_trig.py -- neither the oracle's formula nor the host's long double).
+    The oracle must be within 1e-13; with `_table2` put back to the printed form in fp64 it is not within 1e-11 (periodic axis: 2e-12) -- the
+    cancellation R27 removes is visible at the level of the solve, and this test would catch its return.
+    The z recurrence runs in long double (`zdtype`): with a shift this small the fp64 Thomas elimination itself loses
+    eps / |s| ~ 1e-11 (precision hazards), which would hide what is being pinned; the shift it is given is
+    still the fp64 value of `_table2`.  On a host without 80-bit long double the bounds are the fp64 recurrence's."""
+    import hp_trig
+    n = 2048
+    h = (0.37, 0.37, 0.37)
+    shape = (2, 2, n) if long_axis == "x" else (2, n, 2)
+    bc = (bc_long, N, N) if long_axis == "x" else (N, bc_long, N)          # Neumann mode 0 (constant) on the short axes: lam = 0
+    ks = [1, 2, 3] if bc_long != D else [0, 1, 2]                          # the three lowest non-zero eigenvalues
+    i = np.arange(n)
+    printed_form = lambda theta: -2.0 + 2.0 * np.cos(theta)                # noqa: E731  (the fp64 form R27 replaced)
+    worst_new, worst_old = 0.0, 0.0
+    for k in ks:
+        g = mode_1d(bc_long, n, k)[0]
+        f = np.broadcast_to(g[None, None, :] if long_axis == "x" else g[None, :, None], shape).copy()
+        lam = float(hp_trig.table2_printed(bc_long, k, n)) / h[0] ** 2
+        want = f / lam
+        u = po.solve(f, h, bc, zdtype=np.longdouble)
+        worst_new = max(worst_new, float(np.max(np.abs(u - want)) / np.max(np.abs(want))))
+        with monkeypatch.context() as m:
+            m.setattr(po, "_table2", printed_form)
+            u_old = po.solve(f, h, bc, zdtype=np.longdouble)
+        worst_old = max(worst_old, float(np.max(np.abs(u_old - want)) / np.max(np.abs(want))))
+    if np.finfo(np.longdouble).eps < 2e-19:
+        assert worst_new <= 1e-13, worst_new
+        # (periodic theta = 2 pi k / n is twice the others: the printed form loses four times less there)
+        assert worst_old > (2e-12 if bc_long == P else 1e-11) and worst_old > 20 * worst_new, (worst_old, worst_new)
+    else:
+        assert worst_new <= 3e-11, worst_new
+        assert worst_old > 3 * worst_new, (worst_old, worst_new)
