@@ -415,14 +415,17 @@ def run_cuda(args):
 
     if rank == 0:
         peak, peak_src = measured_peak()
-        # algorithmic bytes per point of each timed slot: 16 per pass; with x+y fusion
-        # the pair's 32 sit in the x slot; the two-level z solve of long lines reads twice (24)
+        # algorithmic bytes per point of each timed slot: 16 per pass, whatever
+        # the number of kernels a slot holds ("so that adding passes cannot inflate it"); with x+y fusion the pair's
+        # 32 sit in the x slot.  What the kernels of a slot actually move is reported beside it: the two-level z solve
+        # of long lines reads its right-hand sides twice (24 B per point).
         slot_bytes = dict.fromkeys(pp.KERNEL_NAMES, BYTES_PER_POINT_KERNEL)
         if paired:
             slot_bytes.update(x_fwd=32.0, y_fwd=0.0, y_inv=0.0, x_inv=32.0)
         xy_launches = 2 if args.fusion else (4 * -(-nz // args.xy_pipeline) if 0 < args.xy_pipeline < nz else 4)
+        moved_bytes = dict(slot_bytes)
         if launches - xy_launches > 2:
-            slot_bytes["z_solve"] = 24.0
+            moved_bytes["z_solve"] = 24.0
         dom = max((k for k in kernel_ms if slot_bytes[k] > 0), key=lambda k: kernel_ms[k] / slot_bytes[k])
         achieved = slot_bytes[dom] * npts / (kernel_ms[dom] * 1e-3) / 1e9
         solve_gbs = BYTES_PER_POINT_SOLVE * npts / (ms_step * 1e-3) / 1e9
@@ -445,7 +448,8 @@ def run_cuda(args):
             "gpu_launches": launches * args.steps,
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "traffic": committed_traffic(wkey, dom), "peak_source": peak_src,
-                         "algorithmic_bytes_per_launch": slot_bytes[dom] * npts},
+                         "algorithmic_bytes_per_launch": slot_bytes[dom] * npts,
+                         "algorithmic_bytes_per_point": slot_bytes[dom], "bytes_moved_per_point": moved_bytes[dom]},
             "roofline_solve": {"bound": "hbm", "achieved": solve_gbs, "peak": peak, "unit": "GB/s",
                                "frac": solve_gbs / peak, "bytes_per_point": BYTES_PER_POINT_SOLVE,
                                "frac_of_nominal_8TBs": solve_gbs / 8000.0},

@@ -112,9 +112,14 @@ int pp_solve_host_batch(pp_plan *plan, const double *f_host, double *u_host, int
  * nbatch independent solves with DEVICE buffers: right-hand side i is the i-th block of nx*ny*nz doubles of f, its
  * solution the i-th block of u (same rules as pp_solve: 16-byte aligned, u == f allowed, no partial overlap).  The
  * transforms of all right-hand sides run as ONE launch per pass (the x and y transforms act on every xy plane
- * independently: a batch is a taller stack of planes), the z solves one after the other:
- * 4 + nbatch (z-solve launches) launches instead of 5 nbatch -- the use the paper itself names is a complex source,
- * "two solves" for its real and imaginary part (reading R17), and small grids stop being launch-bound.
+ * independently: a batch is a taller stack of planes).  The z solves: where the one-CTA partitioned
+ * kernel serves the plan (nz = 32m / 64m <= 512, 1024, 2048; not under PP_Z_SWEEP) up to 64 grids per launch, i.e.
+ * 4 + ceil(nbatch / 64) launches in all; otherwise one z solve after the other, 4 + k nbatch launches with k the
+ * z-solve launches of one pp_solve (pp_plan_launches_per_solve - 4) -- instead of (4 + k) nbatch.  A stack taller
+ * than 65535 planes (the y passes put one plane per blockIdx.y) is cut into groups of floor(65535 / nz) grids, each
+ * group launched as above; any nbatch with nz * nbatch < 2^31 is accepted.  The use the paper itself names is a
+ * complex source, "two solves" for its real and imaginary part (reading R17), and small grids stop
+ * being launch-bound.
  * Stream-ordered, no allocation, no synchronisation.  The x+y fusion / pipeline settings of the plan are ignored.
  */
 int pp_solve_batch(const pp_plan *plan, const double *f, double *u, int nbatch, void *stream);

@@ -209,8 +209,13 @@ def pp_slab_chunk_elems(plan):
 
 
 def pp_slab_set_exchange(plan, fwd_dst, inv_src):
-    """fwd_dst, inv_src: sequences of `world` device addresses."""
+    """fwd_dst, inv_src: sequences of `world` device addresses (the C function reads exactly `world` entries of each)."""
     n = len(fwd_dst)
+    if plan:
+        chunk = pp_slab_chunk_elems(plan)
+        world = pp_slab_local_elems(plan) // chunk if chunk else 0
+        if n != world or len(inv_src) != world:
+            raise ValueError(f"pp_slab_set_exchange: need {world} addresses in fwd_dst and in inv_src, got {n} and {len(inv_src)}")
     a = (ctypes.c_void_p * n)(*[ctypes.c_void_p(int(v)) for v in fwd_dst])
     b = (ctypes.c_void_p * n)(*[ctypes.c_void_p(int(v)) for v in inv_src])
     return lib().pp_slab_set_exchange(ctypes.c_void_p(plan), a, b)

@@ -159,8 +159,20 @@ const char *pp_strerror(int status) {
     }
 }
 
+// ny_z: the number of ky rows the z solve of this plan will see -- ny, or ny / world for the z-side plan of a slab
+// decomposition (its kernel choice and its two-level scratch follow the pencil, not the whole plane)
+static int plan_create_impl(pp_plan **out, int nx, int ny, int nz, double dx, double dy, double dz,
+                            int bc_x, int bc_y, int bc_z, int ny_z);
+
 int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, double dz,
                    int bc_x, int bc_y, int bc_z) {
+    return plan_create_impl(out, nx, ny, nz, dx, dy, dz, bc_x, bc_y, bc_z, ny);
+}
+
+}  // extern "C"
+
+static int plan_create_impl(pp_plan **out, int nx, int ny, int nz, double dx, double dy, double dz,
+                            int bc_x, int bc_y, int bc_z, int ny_z) {
     if (!out) return PP_ERR_NULL;
     *out = nullptr;
     if (nx <= 0 || ny <= 0 || nz <= 0) return PP_ERR_INVALID_ARG;
@@ -222,8 +234,11 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
     // two-level partition (segments of 32 rows; its interface kernels carry the minors over up to 33 rows between
     // renormalisations, hence the range check): interface values [2][nK][plane] + scratch [2][nK][plane], or
     // [6][nK][plane] when the chain of super-segments is cyclic (periodic z)
-    if (!rc && long_ok && zpart_shape(nz).R == 0 && zpart_range_ok(p, 33) && !zpart_cluster(p)) {
-        const size_t nb = sizeof(double) * (bc_z == PP_BC_PERIODIC ? 8 : 4) * (size_t)(nz / ZP_HIER_ROWS) * (size_t)nx * (size_t)ny;
+    p->ny = ny_z;                                  // (the cluster rule looks at the number of lines the z solve sees)
+    const bool z_cluster = zpart_cluster(p);
+    p->ny = ny;
+    if (!rc && long_ok && zpart_shape(nz).R == 0 && zpart_range_ok(p, 33) && !z_cluster) {
+        const size_t nb = sizeof(double) * (bc_z == PP_BC_PERIODIC ? 8 : 4) * (size_t)(nz / ZP_HIER_ROWS) * (size_t)nx * (size_t)ny_z;
         if (cudaMalloc((void **)&p->hier_scratch, nb) != cudaSuccess) { p->hier_scratch = nullptr; cudaGetLastError(); rc = PP_ERR_ALLOC; }
         else p->bytes += nb;
     }
@@ -248,6 +263,8 @@ int pp_plan_create(pp_plan **out, int nx, int ny, int nz, double dx, double dy, 
     *out = p;
     return PP_SUCCESS;
 }
+
+extern "C" {
 
 // a plan's tables live on the device that was current at pp_plan_create: every call that launches must
 // find the same device current (a status code instead of an illegal-address fault at the next sync)
@@ -338,13 +355,22 @@ int pp_solve_batch(const pp_plan *plan, const double *f, double *u, int nbatch, 
         if (a < b + len && b < a + len) return PP_ERR_INVALID_ARG;     // partial overlap
     }
     cudaStream_t st = (cudaStream_t)stream;
-    const int planes = plan->nz * nbatch;
-    int rc;
-    if ((rc = run_x(plan, true, f, u, st, 0, planes))) return rc;          // a1-a3 of every right-hand side
-    if ((rc = run_y_fwd(plan, u, nullptr, st, 0, planes))) return rc;      // a4-a6
-    if ((rc = run_z(plan, u, st, nbatch))) return rc;                      // a7-a8 (up to 64 grids per launch where one CTA holds a line)
-    if ((rc = run_y_inv(plan, u, nullptr, st, 0, planes))) return rc;      // a9
-    return run_x(plan, false, u, u, st, 0, planes);                        // a10
+    // the y passes put one plane per blockIdx.y, and a grid's y extent ends at 65535: the stack is cut into groups of
+    // at most floor(65535 / nz) grids (>= 3, nz <= 16384), each group one launch per transform pass
+    const int group = 65535 / plan->nz;
+    for (int i0 = 0; i0 < nbatch; i0 += group) {
+        const int nb = (nbatch - i0 < group) ? nbatch - i0 : group;
+        const int planes = plan->nz * nb;
+        const double *fg = f + (size_t)i0 * n;
+        double *ug = u + (size_t)i0 * n;
+        int rc;
+        if ((rc = run_x(plan, true, fg, ug, st, 0, planes))) return rc;        // a1-a3 of every right-hand side of the group
+        if ((rc = run_y_fwd(plan, ug, nullptr, st, 0, planes))) return rc;     // a4-a6
+        if ((rc = run_z(plan, ug, st, nb))) return rc;                         // a7-a8 (up to 64 grids per launch where one CTA holds a line)
+        if ((rc = run_y_inv(plan, ug, nullptr, st, 0, planes))) return rc;     // a9
+        if ((rc = run_x(plan, false, ug, ug, st, 0, planes))) return rc;       // a10
+    }
+    return PP_SUCCESS;
 }
 
 int pp_solve_host(pp_plan *plan, const double *f_host, double *u_host, void *stream) {
@@ -375,20 +401,17 @@ int pp_solve_host_batch(pp_plan *plan, const double *f_host, double *u_host, int
     cudaStream_t st = (cudaStream_t)stream;
     const int nstage = nbatch < pp_plan::NSTAGE ? nbatch : pp_plan::NSTAGE;
     // lazily: staging ring, copy streams, events
-    if (!plan->s_in) {
-        if (cudaStreamCreateWithFlags(&plan->s_in, cudaStreamNonBlocking) != cudaSuccess ||
-            cudaStreamCreateWithFlags(&plan->s_out, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
-    }
+    // (each handle is tested on its own, so a creation that failed half-way is completed by the next call instead of
+    // leaving a NULL stream or event in use)
+    for (cudaStream_t *s : {&plan->s_in, &plan->s_out})
+        if (!*s && cudaStreamCreateWithFlags(s, cudaStreamNonBlocking) != cudaSuccess) { *s = nullptr; cudaGetLastError(); return PP_ERR_CUDA; }
     for (int b = 0; b < nstage; ++b) {
         if (!plan->batch_stage[b]) {
             if (cudaMalloc((void **)&plan->batch_stage[b], nb) != cudaSuccess) { plan->batch_stage[b] = nullptr; cudaGetLastError(); return PP_ERR_ALLOC; }
             plan->bytes += nb;
         }
-        if (!plan->ev_in[b]) {
-            if (cudaEventCreateWithFlags(&plan->ev_in[b], cudaEventDisableTiming) != cudaSuccess ||
-                cudaEventCreateWithFlags(&plan->ev_done[b], cudaEventDisableTiming) != cudaSuccess ||
-                cudaEventCreateWithFlags(&plan->ev_out[b], cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return PP_ERR_CUDA; }
-        }
+        for (cudaEvent_t *e : {&plan->ev_in[b], &plan->ev_done[b], &plan->ev_out[b]})
+            if (!*e && cudaEventCreateWithFlags(e, cudaEventDisableTiming) != cudaSuccess) { *e = nullptr; cudaGetLastError(); return PP_ERR_CUDA; }
     }
     // on an error in mid-batch the copies and solves already enqueued still use the staging ring: wait for
     // them before returning, so that a later call cannot reuse a buffer that is in flight
@@ -446,7 +469,7 @@ int pp_slab_plan_create(pp_slab_plan **out, int world, int rank, int nx, int ny,
     std::memset(sp, 0, sizeof(*sp));
     sp->world = world; sp->rank = rank;
     int rc = pp_plan_create(&sp->slab, nx, ny, nz / world, dx, dy, dz, bc_x, bc_y, bc_z);
-    if (!rc) rc = pp_plan_create(&sp->full, nx, ny, nz, dx, dy, dz, bc_x, bc_y, bc_z);
+    if (!rc) rc = plan_create_impl(&sp->full, nx, ny, nz, dx, dy, dz, bc_x, bc_y, bc_z, ny / world);
     if (rc) { free_plan(sp->slab); free_plan(sp->full); delete sp; return rc; }
     const int nyl = ny / world;
     sp->zview = *sp->full;                       // shares full's device tables; owns nothing
@@ -535,12 +558,12 @@ int pp_plan_set_xy_pipeline(pp_plan *plan, int planes_per_slab) {
     if (int rc = check_device(plan)) return rc;
     if (planes_per_slab > 0) {
         if ((plan->nz + planes_per_slab - 1) / planes_per_slab > pp_plan::MAX_PIPE) return PP_ERR_INVALID_ARG;
-        if (!plan->pipe) {
-            if (cudaStreamCreateWithFlags(&plan->pipe, cudaStreamNonBlocking) != cudaSuccess) { plan->pipe = nullptr; cudaGetLastError(); return PP_ERR_CUDA; }
-            for (auto &e : plan->ev_pipe)
-                if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) { e = nullptr; cudaGetLastError(); return PP_ERR_CUDA; }
-            if (cudaEventCreateWithFlags(&plan->ev_pipe_join, cudaEventDisableTiming) != cudaSuccess) { plan->ev_pipe_join = nullptr; cudaGetLastError(); return PP_ERR_CUDA; }
-        }
+        // each handle tested on its own: a creation that failed half-way is completed by the next call, and the
+        // pipeline is only switched on (below) once every stream and event exists
+        if (!plan->pipe && cudaStreamCreateWithFlags(&plan->pipe, cudaStreamNonBlocking) != cudaSuccess) { plan->pipe = nullptr; cudaGetLastError(); return PP_ERR_CUDA; }
+        for (auto &e : plan->ev_pipe)
+            if (!e && cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) { e = nullptr; cudaGetLastError(); return PP_ERR_CUDA; }
+        if (!plan->ev_pipe_join && cudaEventCreateWithFlags(&plan->ev_pipe_join, cudaEventDisableTiming) != cudaSuccess) { plan->ev_pipe_join = nullptr; cudaGetLastError(); return PP_ERR_CUDA; }
     }
     plan->xy_pipeline = planes_per_slab;
     return PP_SUCCESS;

@@ -247,3 +247,82 @@ def test_solve_batch_is_the_solves_one_by_one(shape, combo):
     with pytest.raises(ValueError):
         plan.solve_batch(ft[0])
     plan.destroy()
+
+
+@pytest.mark.parametrize("nb", [65, 130])
+def test_solve_batch_beyond_one_z_launch(nb):
+    """More right-hand sides than one launch of the batched z kernel takes (64, Z_MAX_BATCH in csrc/pp_zshape.h): every
+    solution against the oracle, and bit-identical to a pp_solve of its own."""
+    import numpy as np
+    import torch
+    import paper_1909_05423_b200 as pp
+    from oracle import poisson_oracle as po
+    from paper_1909_05423_b200 import workloads as wl
+    shape, bc = (32, 32, 32), wl.parse_bc("PPN")                    # singular: every grid gets its own zero-mode line
+    h = (1.0 / 32, 0.7 / 32, 1.3 / 32)
+    f = np.stack([wl.random_normal(shape, 2000 + i, zero_mean=False) for i in range(nb)])
+    plan = pp.Plan(32, 32, 32, *h, bc)
+    ft = torch.from_numpy(f).cuda()
+    ub = plan.solve_batch(ft)
+    torch.cuda.synchronize()
+    got = ub.cpu().numpy()
+    for i in range(nb):
+        assert rel_err(got[i], po.solve(f[i], h, bc)) <= TOL, i
+    for i in (0, 63, 64, nb - 1):
+        assert torch.equal(plan.solve(ft[i].contiguous()), ub[i]), i
+    plan.destroy()
+
+
+@pytest.mark.parametrize("shape,combo", [((768, 8, 8), "PPP"), ((768, 128, 256), "NND"), ((768, 128, 256), "NNN"), ((512, 16, 8), "PPN")])
+def test_solve_batch_on_long_lines(shape, combo):
+    """Three right-hand sides where the z solve is not the one-CTA kernel: the two-level partition (8 x 8 x 768, cyclic;
+    8 x 16 x 512 takes the one-CTA kernel with 64 rows per thread) and the cluster kernel (256 x 128 x 768), each against
+    the oracle."""
+    import numpy as np
+    import torch
+    import paper_1909_05423_b200 as pp
+    from oracle import poisson_oracle as po
+    from paper_1909_05423_b200 import workloads as wl
+    bc = wl.parse_bc(combo)
+    nz, ny, nx = shape
+    h = (1.0 / nx, 0.7 / ny, 1.3 / nz)
+    f = np.stack([wl.random_normal(shape, 3000 + i, zero_mean=False) for i in range(3)])
+    plan = pp.Plan(nx, ny, nz, *h, bc)
+    ft = torch.from_numpy(f).cuda()
+    ub = plan.solve_batch(ft)
+    torch.cuda.synchronize()
+    got = ub.cpu().numpy()
+    for i in range(3):
+        assert rel_err(got[i], po.solve(f[i], h, bc)) <= TOL, i
+        assert torch.equal(plan.solve(ft[i].contiguous()), ub[i]), i
+    plan.destroy()
+
+
+@pytest.mark.parametrize("shape,combo,nb", [((8, 8, 8), "NNN", 8200), ((256, 4, 4), "PPD", 257), ((16384, 4, 4), "DDN", 5)])
+def test_solve_batch_taller_than_one_grid(shape, combo, nb):
+    """nz * nbatch > 65535 planes: more than the y extent of one launch grid (the y passes put a plane on blockIdx.y), so
+    the stack is solved in groups of floor(65535 / nz) grids.  Sampled solutions against the oracle -- the last grid of a
+    group, the first of the next, the very last -- and the whole stack against the same stack solved in two halves."""
+    import numpy as np
+    import torch
+    import paper_1909_05423_b200 as pp
+    from oracle import poisson_oracle as po
+    from paper_1909_05423_b200 import workloads as wl
+    bc = wl.parse_bc(combo)
+    nz, ny, nx = shape
+    assert nz * nb > 65535
+    h = (1.0 / nx, 0.7 / ny, 1.3 / nz) if nz <= 256 else (0.02, 0.03, 0.025)    # long lines: keep dz / dx of order one
+    rng = np.random.default_rng(4000 + nb)
+    f = rng.standard_normal((nb,) + shape)
+    plan = pp.Plan(nx, ny, nz, *h, bc)
+    ft = torch.from_numpy(f).cuda()
+    ub = plan.solve_batch(ft)
+    torch.cuda.synchronize()
+    group = 65535 // nz
+    for i in sorted({0, group - 1, group, min(2 * group, nb - 1), nb - 1}):
+        assert rel_err(ub[i].cpu().numpy(), po.solve(f[i], h, bc)) <= TOL, i
+    half = nb // 2
+    two = torch.cat([plan.solve_batch(ft[:half].contiguous()), plan.solve_batch(ft[half:].contiguous())])
+    torch.cuda.synchronize()
+    assert torch.equal(two, ub)
+    plan.destroy()

@@ -50,6 +50,19 @@ def test_virtual_ranks_other_shapes(shape, world):
         assert np.array_equal(u, gpu_solve(f, h, bc))
 
 
+@pytest.mark.parametrize("world", [2, 4])
+def test_virtual_ranks_long_lines_follow_the_pencil(world):
+    """nz = 768 on a 256 x 256 plane: the whole grid takes the cluster z kernel; a pencil of 256 x 128 lines still does,
+    one of 256 x 64 lines is below the cluster rule's line count and takes the two-level partition, whose scratch the
+    slab plan sizes for the pencil (it used to fall back to the two-sweep kernel: no scratch had been allocated)."""
+    shape, h = (768, 256, 256), (0.02, 0.03, 0.025)
+    for combo in ("NND", "NNN"):
+        bc = wl.parse_bc(combo)
+        f = wl.random_normal(shape, 78, zero_mean=all(b in (0, 1) for b in bc))
+        u = slab_solve(f, h, bc, world)
+        assert rel_err(u, po.solve(f, h, bc)) <= TOL
+
+
 def test_slab_plan_argument_checks():
     import paper_1909_05423_b200 as pp
     from paper_1909_05423_b200 import binding as b
@@ -62,4 +75,6 @@ def test_slab_plan_argument_checks():
     x = torch.zeros(16, 32, 32, dtype=torch.float64, device="cuda")
     with pytest.raises(pp.PittPackError):
         p.forward(x, x)                                                                   # exchange addresses not set
+    with pytest.raises(ValueError):
+        p.set_exchange([x.data_ptr()], [x.data_ptr()])                                    # one address for world = 2
     p.destroy()
