@@ -319,7 +319,9 @@ def run_cuda(args):
     # ---- timed region: K solves, inputs resident in HBM (f, u: 2 x N x 8 B, far larger than L2)
     sampler = ClockSampler(physical_gpu_index(local_rank))
     sampler.start()
-    time.sleep(0.05)
+    t_wait = time.perf_counter()                        # NVML start-up can take longer than a short timed region:
+    while sampler.mark() < 3 and not getattr(sampler, "error", None) and time.perf_counter() - t_wait < 10.0:
+        time.sleep(0.005)                               # wait for the first samples, not for a fixed time
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     m0 = sampler.mark()
@@ -354,6 +356,26 @@ def run_cuda(args):
             gs.synchronize()
         graph_ms = g0.elapsed_time(g1) / args.steps
         del graph
+
+    # ---- many right-hand sides as one stack (pp_solve_batch): the launch-bound grids at the large grids' speed
+    batch = None
+    if args.batch > 1 and world == 1:
+        fb = f.unsqueeze(0).repeat(args.batch, 1, 1, 1).contiguous()
+        ub = torch.empty_like(fb)
+        for _ in range(3):
+            plan.solve_batch(fb, ub)
+        b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        b0.record(stream)
+        for _ in range(args.steps):
+            plan.solve_batch(fb, ub)
+        b1.record(stream)
+        torch.cuda.synchronize()
+        bms = b0.elapsed_time(b1) / args.steps
+        batch = {"api": "pp_solve_batch", "right_hand_sides": args.batch, "ms_per_batch": bms,
+                 "value": args.batch * npts / (bms * 1e-3) / 1e9, "unit": UNIT,
+                 "one_by_one_ms": ms_step * args.batch, "bit_identical_to_single_solves": bool(torch.equal(ub[args.batch - 1], u))}
+        del fb, ub
 
     # ---- per-kernel durations over the same number of steps (CUDA events on the launching stream)
     plan.set_profiling(True)
@@ -456,6 +478,7 @@ def run_cuda(args):
             "kernel_ms": kernel_ms,
             "kernel_gbs": {k: slot_bytes[k] * npts / (v * 1e-3) / 1e9 for k, v in kernel_ms.items() if slot_bytes[k] > 0},
             "graph_replay_ms_per_step": graph_ms,
+            "batch": batch,
             "check": {"sampled_residual_rel": residual,
                       "what": "max|A u - f| / max|f| at 200000 random cells of the last timed solve's output (eq. 3)"},
         }
@@ -482,50 +505,6 @@ def run_cuda(args):
         dist.destroy_process_group()
     return 0
 
-
-
-def run_probe_l2(args):
-    """SM-side throughput of the five passes with HBM out of the way: S streams, each with its own plan, solve the SAME
-    slab of the workload's x-y extent in place at the same time (a deliberate race: timing only).  The slab (<= 64 MiB)
-    stays in L2; enough CTAs are in flight to fill the machine.  Compare `equivalent_ms` with the HBM-fed solve."""
-    import torch
-    import paper_1909_05423_b200 as pp
-    w = workload_by_name(args.workload, args.bc)
-    nz, ny, nx = w.shape
-    nzs = 32
-    while nzs > 2 and nx * ny * nzs * 8 > (64 << 20):
-        nzs //= 2
-    torch.cuda.set_device(0)
-    out = {"probe": "l2_resident_concurrent_solves", "workload": describe(w), "slab": f"{nx}x{ny}x{nzs}",
-           "slab_mib": nx * ny * nzs * 8 / 2 ** 20, "runs": []}
-    for nstreams in (1, 4, 8):
-        plans = [pp.Plan(nx, ny, nzs, *w.h, w.bc) for _ in range(nstreams)]
-        u = torch.randn(nzs, ny, nx, dtype=torch.float64, device="cuda")
-        streams = [torch.cuda.Stream() for _ in range(nstreams)]
-        def go(n):
-            for _ in range(n):
-                for p, st in zip(plans, streams):
-                    p.solve(u, u, stream=st)
-        go(3)
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        cur = torch.cuda.current_stream()
-        e0.record(cur)
-        for st in streams:
-            st.wait_stream(cur)
-        go(args.steps)
-        for st in streams:
-            cur.wait_stream(st)
-        e1.record(cur)
-        torch.cuda.synchronize()
-        ms = e0.elapsed_time(e1)
-        pts = nx * ny * nzs * nstreams * args.steps
-        out["runs"].append({"streams": nstreams, "gpoints_per_s": pts / ms / 1e6,
-                            "equivalent_ms": ms * w.n_points / pts})
-        for p in plans:
-            p.destroy()
-    print(json.dumps(out))
-    return 0
 
 
 def spawn_ranks(args):
@@ -555,11 +534,10 @@ def main():
     ap.add_argument("--lib", default=None, metavar="PATH",
                     help="load this build of the library instead of the default one (a variant built with "
                          "`python -m paper_1909_05423_b200.build -D... -o PATH`: tuning switches of the kernels)")
+    ap.add_argument("--batch", type=int, default=0, metavar="NB",
+                    help="also time pp_solve_batch on NB copies of the workload's right-hand side (adds a `batch` key)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer (e2e) legs: for runs under a profiler")
-    ap.add_argument("--probe-l2", action="store_true",
-                    help="instead of the benchmark: SM-side throughput probe -- several streams solve one L2-resident "
-                         "slab of the workload's x-y extent in place at the same time (DESIGN.md section 9)")
     args = ap.parse_args()
     if args.bc is not None and (len(args.bc) != 3 or any(c not in "PNDpnd" for c in args.bc)):
         raise SystemExit("--bc: three letters out of P, N, D")
@@ -568,8 +546,6 @@ def main():
         binding.LIB_PATH = os.path.abspath(args.lib)
     if args.impl == "reference":
         return run_reference(args)
-    if args.probe_l2:
-        return run_probe_l2(args)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         return spawn_ranks(args)
     return run_cuda(args)

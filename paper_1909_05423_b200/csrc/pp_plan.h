@@ -13,7 +13,18 @@ namespace pp {
 struct YRows;
 }
 
+// Tensor maps of the y passes (pp_tma.cuh) hold the address of the array they describe: they are encoded on the host, by
+// the driver, and kept here per direction for as long as the same array, plane count and boundary condition come back --
+// the usual case (a caller solving in the same buffers) then pays no cuTensorMapEncodeTiled on its launch path.
+// `maps` is a YTmaMaps (pp_ypass.cuh; three CUtensorMap of 128 bytes, 64-byte aligned), opaque here.
+struct alignas(64) YMapSlot {
+    unsigned char maps[3 * 128];
+    const void *w;             // array the maps describe (NULL: empty slot)
+    int planes, bc;
+};
+
 struct pp_plan {
+    YMapSlot ymap[2];          // [0] forward, [1] inverse y pass
     int nx, ny, nz;
     double dx, dy, dz;
     int bcx, bcy, bcz;

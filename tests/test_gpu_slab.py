@@ -78,3 +78,38 @@ def test_slab_plan_argument_checks():
     with pytest.raises(ValueError):
         p.set_exchange([x.data_ptr()], [x.data_ptr()])                                    # one address for world = 2
     p.destroy()
+
+
+@pytest.mark.parametrize("combo", ["PPN", "NND", "NNN"])
+def test_two_processes_one_gpu_peer_pointers_over_cuda_ipc(combo):
+    """The multi-process form of the decomposed solve, on the one GPU there is: two processes, each with its own SlabPlan
+    and its own pencil, the pencils exported to each other by CUDA IPC and used as the peer addresses of the fused y
+    passes (tests/slab_ipc_worker.py).  Element-wise against the oracle."""
+    import torch.multiprocessing as mp
+    import slab_ipc_worker
+    world, shape, h = 2, (32, 64, 128), (1.0 / 128, 1.0 / 64, 1.0 / 32)
+    bc = wl.parse_bc(combo)
+    f = wl.random_normal(shape, 4300, zero_mean=all(b in (0, 1) for b in bc))
+    ctx = mp.get_context("spawn")
+    queues = [ctx.Queue() for _ in range(world)]
+    results, barrier = ctx.Queue(), ctx.Barrier(world)
+    nzl = shape[0] // world
+    procs = [ctx.Process(target=slab_ipc_worker.run_rank,
+                         args=(r, world, (shape[2], shape[1], shape[0]), h, bc, np.ascontiguousarray(f[r * nzl:(r + 1) * nzl]),
+                               queues, barrier, results)) for r in range(world)]
+    for p in procs:
+        p.start()
+    try:
+        got = {}
+        for _ in range(world):
+            rank, u, err = results.get(timeout=300)
+            assert err is None, f"rank {rank}:\n{err}"
+            got[rank] = u
+    finally:
+        for p in procs:
+            p.join(timeout=60)
+            if p.is_alive():
+                p.kill()                      # exactly the process started here
+    u = np.concatenate([got[r] for r in range(world)])
+    assert rel_err(u, po.solve(f, h, bc)) <= TOL
+    assert np.array_equal(u, gpu_solve(f, h, bc))                       # identical to the undecomposed solve
